@@ -1,0 +1,510 @@
+// ens_oracle.cpp — CPU ORACLE for the ensemble Hermite / MVS step loop of Swarm-NG (arxiv 1208.1157).
+//
+// THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may build, load or call anything under oracle/.  It shares no code
+// (headers, helpers, tables, constants) with paper_1208_1157_b200/csrc and neither side includes the other.
+//
+// Plain, slow, one system at a time, IEEE double (prec=0) or x87 80-bit long double (prec=1, the noise
+// reference), correctly rounded sqrt and divide, no fast-math, compiled with -ffp-contract=off.
+// It follows PAPER.md (`P:L<n>` = /root/reference/PAPER.md line n) step by step, with the readings
+// R1..R15, R-M1..R-M7 of DESIGN.md §3 where the extracted text is garbled or silent.
+//
+// Layout of every array argument: C order, pos/vel [n_sys][n_body][3], mass [n_sys][n_body], per-system
+// arrays [n_sys].  Body 0 is the central body.  G = 1.
+//
+// Pins (tests/test_oracle_*.py): 2-body closed forms, Kepler's equation, order-4 / order-2 convergence,
+// symmetric-corrector identity, reversal, invariants, finite-difference jerk, brute-force sums, Stumpff
+// closed forms, test-particle exactness of the Kepler drift, hand-built monitor crossings.  No function
+// in this file is "parity unpinned"; the only unpinned item is the paper's Table 1, whose
+// orbital phases are unspecified.
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+
+namespace {
+
+enum { ST_ACTIVE = 0, ST_DONE_TIME = 1, ST_DONE_STEPS = 2, ST_STOP_CLOSE = 3, ST_STOP_EJECT = 4, ST_STOP_NONFINITE = 5 };
+
+template <class R> inline R rsqrt_exact(R r2) { return R(1) / std::sqrt(r2); }
+
+// ---------------------------------------------------------------------------------------------------
+// Acceleration and jerk.  Eq. 1 (denominator read as |x_j - x_i|^3, R1) and its time derivative
+// ("analytic expressions", R2):   a_i = sum_k m_k dx / r^3,   j_i = sum_k m_k [dv/r^3 - 3 (dx.dv) dx / r^5].
+// Summation order: planets k = 1..n-1 ascending, the star (body 0) LAST (R7).
+// ---------------------------------------------------------------------------------------------------
+template <class R>
+void eval_acc_jerk(int n, const R* x, const R* v, const R* m, R* a, R* j) {
+    for (int i = 0; i < n; ++i) {
+        R ai[3] = {0, 0, 0}, ji[3] = {0, 0, 0};
+        for (int kk = 1; kk <= n; ++kk) {
+            const int k = (kk == n) ? 0 : kk;  // 1, 2, ..., n-1, then 0
+            if (k == i) continue;
+            R dx[3], dv[3];
+            for (int c = 0; c < 3; ++c) {
+                dx[c] = x[3 * k + c] - x[3 * i + c];
+                dv[c] = v[3 * k + c] - v[3 * i + c];
+            }
+            const R r2 = dx[0] * dx[0] + dx[1] * dx[1] + dx[2] * dx[2];
+            const R rv = dx[0] * dv[0] + dx[1] * dv[1] + dx[2] * dv[2];
+            const R rinv = rsqrt_exact(r2);
+            const R rinv3 = rinv * rinv * rinv;
+            for (int c = 0; c < 3; ++c) {
+                ai[c] += m[k] * rinv3 * dx[c];
+                ji[c] += m[k] * rinv3 * (dv[c] - R(3) * (rv / r2) * dx[c]);
+            }
+        }
+        for (int c = 0; c < 3; ++c) {
+            a[3 * i + c] = ai[c];
+            j[3 * i + c] = ji[c];
+        }
+    }
+}
+
+// Acceleration only, planets on planets, in heliocentric positions Q (index 1..n-1); the star-planet
+// term is excluded because the Kepler drift carries it.
+template <class R>
+void eval_acc_planets(int n, const R* Q, const R* m, R* A) {
+    for (int i = 1; i < n; ++i) {
+        R ai[3] = {0, 0, 0};
+        for (int k = 1; k < n; ++k) {
+            if (k == i) continue;
+            R dx[3];
+            for (int c = 0; c < 3; ++c) dx[c] = Q[3 * k + c] - Q[3 * i + c];
+            const R r2 = dx[0] * dx[0] + dx[1] * dx[1] + dx[2] * dx[2];
+            const R rinv = rsqrt_exact(r2);
+            const R rinv3 = rinv * rinv * rinv;
+            for (int c = 0; c < 3; ++c) ai[c] += m[k] * rinv3 * dx[c];
+        }
+        for (int c = 0; c < 3; ++c) A[3 * i + c] = ai[c];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// One Hermite step, Alg. 2 with Eq. 3 and Eq. 4 read as R3-R6:
+//   three evaluations per step: (a0,j0) at the current state, then two corrector iterations
+//   (P:L89), each re-evaluating (a_k,j_k) at the latest iterate; corrector base is the PREDICTED x_p,v_p,
+//   coefficient of (a0-a_k) h^2 is 3/20.
+// ---------------------------------------------------------------------------------------------------
+template <class R>
+void hermite_step(int n, R* x, R* v, const R* m, R h, int n_corr = 2) {
+    const int d = 3 * n;
+    std::vector<R> a0(d), j0(d), a1(d), j1(d), xp(d), vp(d), xc(d), vc(d);
+    eval_acc_jerk(n, x, v, m, a0.data(), j0.data());
+    for (int q = 0; q < d; ++q) {
+        xp[q] = x[q] + v[q] * h + a0[q] * (h * h) / R(2) + j0[q] * (h * h * h) / R(6);
+        vp[q] = v[q] + a0[q] * h + j0[q] * (h * h) / R(2);
+        xc[q] = xp[q];
+        vc[q] = vp[q];
+    }
+    for (int it = 0; it < n_corr; ++it) {
+        eval_acc_jerk(n, xc.data(), vc.data(), m, a1.data(), j1.data());
+        for (int q = 0; q < d; ++q) {
+            xc[q] = xp[q] - (R(3) / R(20)) * (a0[q] - a1[q]) * (h * h) - (R(1) / R(60)) * (R(7) * j0[q] + R(2) * j1[q]) * (h * h * h);
+            vc[q] = vp[q] - (R(1) / R(2)) * (a0[q] - a1[q]) * h - (R(1) / R(12)) * (R(5) * j0[q] + j1[q]) * (h * h);
+        }
+    }
+    for (int q = 0; q < d; ++q) {
+        x[q] = xc[q];
+        v[q] = vc[q];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Monitors (Alg. 1 `execute(M)` after `advance(P)`; thresholds from BASELINE.json;
+// reading R11).  Evaluated on the post-step state only.  Order: non-finite, close approach, ejection.
+// ---------------------------------------------------------------------------------------------------
+template <class R>
+int monitors(int n, const R* x, double r_close, double r_eject) {
+    for (int i = 0; i < n; ++i) {
+        const R d2 = x[3 * i] * x[3 * i] + x[3 * i + 1] * x[3 * i + 1] + x[3 * i + 2] * x[3 * i + 2];
+        if (!std::isfinite((double)d2)) return ST_STOP_NONFINITE;
+    }
+    if (r_close > 0) {
+        for (int i = 0; i < n; ++i)
+            for (int k = i + 1; k < n; ++k) {
+                R dx[3];
+                for (int c = 0; c < 3; ++c) dx[c] = x[3 * k + c] - x[3 * i + c];
+                const R r = std::sqrt(dx[0] * dx[0] + dx[1] * dx[1] + dx[2] * dx[2]);
+                if (r < R(r_close)) return ST_STOP_CLOSE;
+            }
+    }
+    if (std::isfinite(r_eject) && r_eject > 0) {
+        for (int i = 0; i < n; ++i) {
+            const R d = std::sqrt(x[3 * i] * x[3 * i] + x[3 * i + 1] * x[3 * i + 1] + x[3 * i + 2] * x[3 * i + 2]);
+            if (d > R(r_eject)) return ST_STOP_EJECT;
+        }
+    }
+    return ST_ACTIVE;
+}
+
+inline bool time_left(double dt, double t, double t_end) {
+    // direction-aware `t < t_end` (R10): continue while sign(dt) * (t_end - t) > 0; no clipping of the last step.
+    return dt > 0 ? (t < t_end) : (t > t_end);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Energy and angular momentum.  Eq. 6 with each unordered pair counted once (R9).
+// ---------------------------------------------------------------------------------------------------
+template <class R>
+void energy_L(int n, const R* x, const R* v, const R* m, R* E, R* L) {
+    R ke = 0, pe = 0;
+    for (int i = 0; i < n; ++i) ke += R(0.5) * m[i] * (v[3 * i] * v[3 * i] + v[3 * i + 1] * v[3 * i + 1] + v[3 * i + 2] * v[3 * i + 2]);
+    for (int i = 0; i < n; ++i)
+        for (int k = i + 1; k < n; ++k) {
+            R dx[3];
+            for (int c = 0; c < 3; ++c) dx[c] = x[3 * k + c] - x[3 * i + c];
+            pe -= m[i] * m[k] / std::sqrt(dx[0] * dx[0] + dx[1] * dx[1] + dx[2] * dx[2]);
+        }
+    *E = ke + pe;
+    if (L) {
+        L[0] = L[1] = L[2] = 0;
+        for (int i = 0; i < n; ++i) {
+            const R* xi = x + 3 * i;
+            const R* vi = v + 3 * i;
+            L[0] += m[i] * (xi[1] * vi[2] - xi[2] * vi[1]);
+            L[1] += m[i] * (xi[2] * vi[0] - xi[0] * vi[2]);
+            L[2] += m[i] * (xi[0] * vi[1] - xi[1] * vi[0]);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Stumpff functions c0..c3 (c_n(z) = sum_k (-z)^k / (2k+n)!): series for |z| small, argument quartering
+// otherwise (R-M3).  c0 = cos sqrt z, c1 = sin sqrt z / sqrt z, c2 = (1-c0)/z, c3 = (1-c1)/z for z > 0.
+// ---------------------------------------------------------------------------------------------------
+template <class R>
+void stumpff(R z, R c[4]) {
+    int nq = 0;
+    while (std::fabs(z) > R(0.1)) {
+        z /= R(4);
+        ++nq;
+    }
+    // series c_n(z) = sum_k (-z)^k / (2k+n)!, 12 terms: |z|^12 / 26! is far below 1e-30 for |z| <= 0.1
+    R t2 = R(1) / R(2), t3 = R(1) / R(6);  // k = 0 terms: 1/2!, 1/3!
+    R c2 = t2, c3 = t3;
+    for (int k = 1; k < 12; ++k) {
+        t2 *= -z / R((2 * k + 1) * (2 * k + 2));
+        t3 *= -z / R((2 * k + 2) * (2 * k + 3));
+        c2 += t2;
+        c3 += t3;
+    }
+    R c1 = R(1) - z * c3;
+    R c0 = R(1) - z * c2;
+    for (; nq > 0; --nq) {
+        // c_n(4z) from c_n(z)
+        const R n3 = (c2 + c0 * c3) / R(4);
+        const R n2 = c1 * c1 / R(2);
+        const R n1 = c0 * c1;
+        const R n0 = R(2) * c0 * c0 - R(1);
+        c3 = n3; c2 = n2; c1 = n1; c0 = n0;
+    }
+    c[0] = c0; c[1] = c1; c[2] = c2; c[3] = c3;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Kepler drift of one body about a fixed centre of gravitational parameter mu for time tau,
+// by universal variables (BASELINE.json config 4; R-M3, R-M4):
+//   r0 = |q|, eta = q.p, beta = 2 mu / r0 - |p|^2;   solve  r0 G1 + eta G2 + mu G3 = tau  for X,
+//   G_n = X^n c_n(beta X^2); Newton with derivative r = r0 G0 + eta G1 + mu G2; guess X = tau / r0.
+//   f = 1 - mu G2 / r0, g = tau - mu G3, f' = -mu G1 / (r0 r), g' = 1 - mu G2 / r.
+// Returns the number of Newton iterations (negative if the bisection fallback was needed).
+// ---------------------------------------------------------------------------------------------------
+template <class R>
+struct GFun { R G0, G1, G2, G3; };
+
+template <class R>
+GFun<R> gfuncs(R beta, R X) {
+    R c[4];
+    stumpff(beta * X * X, c);
+    GFun<R> G;
+    G.G0 = c[0];
+    G.G1 = X * c[1];
+    G.G2 = X * X * c[2];
+    G.G3 = X * X * X * c[3];
+    return G;
+}
+
+template <class R>
+int kepler_drift(R* q, R* p, R mu, R tau) {
+    const R r0 = std::sqrt(q[0] * q[0] + q[1] * q[1] + q[2] * q[2]);
+    const R eta = q[0] * p[0] + q[1] * p[1] + q[2] * p[2];
+    const R v2 = p[0] * p[0] + p[1] * p[1] + p[2] * p[2];
+    const R beta = R(2) * mu / r0 - v2;
+    const R eps = std::is_same<R, double>::value ? R(1e-15) : R(1e-18);
+
+    auto resid = [&](R X, GFun<R>& G) {
+        G = gfuncs(beta, X);
+        return r0 * G.G1 + eta * G.G2 + mu * G.G3 - tau;
+    };
+
+    R X = tau / r0;
+    GFun<R> G;
+    int iters = 0;
+    bool ok = false;
+    for (; iters < 50; ++iters) {
+        const R F = resid(X, G);
+        const R dF = r0 * G.G0 + eta * G.G1 + mu * G.G2;
+        const R dX = F / dF;
+        X -= dX;
+        if (!(std::fabs(dX) > eps * std::fabs(X))) { ok = true; ++iters; break; }
+    }
+    if (!ok || !std::isfinite((double)X)) {
+        // guaranteed-convergent fallback: the residual is monotone in X (dF/dX = r > 0); bracket and bisect.
+        R lo = 0, hi = tau / r0;
+        GFun<R> Gt;
+        const R sgn = tau >= 0 ? R(1) : R(-1);
+        if (hi == 0) hi = sgn;
+        for (int k = 0; k < 200 && sgn * resid(hi, Gt) < 0; ++k) hi *= R(2);
+        for (int k = 0; k < 200; ++k) {
+            const R mid = R(0.5) * (lo + hi);
+            if (sgn * resid(mid, Gt) < 0) lo = mid; else hi = mid;
+        }
+        X = R(0.5) * (lo + hi);
+        iters = -iters;
+    }
+    G = gfuncs(beta, X);
+    const R r = r0 * G.G0 + eta * G.G1 + mu * G.G2;
+    const R f = R(1) - mu * G.G2 / r0;
+    const R g = tau - mu * G.G3;
+    const R fd = -mu * G.G1 / (r0 * r);
+    const R gd = R(1) - mu * G.G2 / r;
+    for (int c = 0; c < 3; ++c) {
+        const R qn = f * q[c] + g * p[c];
+        const R pn = fd * q[c] + gd * p[c];
+        q[c] = qn;
+        p[c] = pn;
+    }
+    return iters;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// MVS in democratic-heliocentric variables (R-M1): heliocentric positions Q_i = x_i - x_0, barycentric
+// velocities V_i = v_i - V_cm (i >= 1), plus the centre of mass X_cm, V_cm.  Five sub-steps, unmerged
+// (R-M7); mu = G m_0 (R-M2); planet-planet accelerations reused across the step boundary.
+// ---------------------------------------------------------------------------------------------------
+template <class R>
+struct DH {
+    int n;
+    std::vector<R> Q, V, A;  // index 3*i+c, i = 1..n-1 (slot 0 unused)
+    R Xcm[3], Vcm[3], M;
+};
+
+template <class R>
+void to_dh(int n, const R* x, const R* v, const R* m, DH<R>& s) {
+    s.n = n;
+    s.Q.assign(3 * n, 0); s.V.assign(3 * n, 0); s.A.assign(3 * n, 0);
+    s.M = 0;
+    for (int i = 0; i < n; ++i) s.M += m[i];
+    for (int c = 0; c < 3; ++c) {
+        R sx = 0, sv = 0;
+        for (int i = 0; i < n; ++i) { sx += m[i] * x[3 * i + c]; sv += m[i] * v[3 * i + c]; }
+        s.Xcm[c] = sx / s.M;
+        s.Vcm[c] = sv / s.M;
+    }
+    for (int i = 1; i < n; ++i)
+        for (int c = 0; c < 3; ++c) {
+            s.Q[3 * i + c] = x[3 * i + c] - x[c];
+            s.V[3 * i + c] = v[3 * i + c] - s.Vcm[c];
+        }
+}
+
+template <class R>
+void from_dh(const DH<R>& s, const R* m, R* x, R* v) {
+    const int n = s.n;
+    for (int c = 0; c < 3; ++c) {
+        R sq = 0, sp = 0;
+        for (int k = 1; k < n; ++k) { sq += m[k] * s.Q[3 * k + c]; sp += m[k] * s.V[3 * k + c]; }
+        x[c] = s.Xcm[c] - sq / s.M;
+        if (v) v[c] = s.Vcm[c] - sp / m[0];
+        for (int i = 1; i < n; ++i) {
+            x[3 * i + c] = x[c] + s.Q[3 * i + c];
+            if (v) v[3 * i + c] = s.V[3 * i + c] + s.Vcm[c];
+        }
+    }
+}
+
+template <class R>
+void mvs_linear_drift(DH<R>& s, const R* m, R hh) {  // Cartesian drift
+    for (int c = 0; c < 3; ++c) {
+        R sp = 0;
+        for (int k = 1; k < s.n; ++k) sp += m[k] * s.V[3 * k + c];
+        const R sh = sp / m[0];
+        for (int i = 1; i < s.n; ++i) s.Q[3 * i + c] += hh * sh;
+        s.Xcm[c] += hh * s.Vcm[c];
+    }
+}
+
+template <class R>
+void mvs_kick(DH<R>& s, R hh) {
+    for (int q = 3; q < 3 * s.n; ++q) s.V[q] += hh * s.A[q];
+}
+
+template <class R>
+void mvs_step(DH<R>& s, const R* m, R h) {
+    const R hh = h / R(2);
+    mvs_linear_drift(s, m, hh);
+    mvs_kick(s, hh);
+    for (int i = 1; i < s.n; ++i) kepler_drift(&s.Q[3 * i], &s.V[3 * i], m[0], h);
+    eval_acc_planets(s.n, s.Q.data(), m, s.A.data());
+    mvs_kick(s, hh);
+    mvs_linear_drift(s, m, hh);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// The generic integrator loop, Alg. 1 with R10-R12:
+//   while ACTIVE and steps_this_call < max_steps and time left: advance; ++nsteps; t += h; monitors;
+//   exit status: STOP_* (sticky) | DONE_TIME (t reached t_end) | DONE_STEPS.
+// ---------------------------------------------------------------------------------------------------
+template <class R>
+void run_system(int integrator, int n, double* pos, double* vel, const double* mass, double* time, int32_t* status,
+                int64_t* nsteps, double dt, double t_end, int64_t max_steps, double r_close, double r_eject, int n_corr) {
+    if (*status >= ST_STOP_CLOSE) return;  // sticky until the state is set again
+    std::vector<R> x(3 * n), v(3 * n), m(n);
+    for (int q = 0; q < 3 * n; ++q) { x[q] = pos[q]; v[q] = vel[q]; }
+    for (int i = 0; i < n; ++i) m[i] = mass[i];
+    R t = *time;
+    const R h = dt;
+    int st = ST_ACTIVE;
+    int64_t k = 0;
+    DH<R> s;
+    std::vector<R> xm(3 * n);
+    if (integrator == 1) {
+        to_dh(n, x.data(), v.data(), m.data(), s);
+        eval_acc_planets(n, s.Q.data(), m.data(), s.A.data());  // prepare(P)
+    }
+    while (true) {
+        if (!time_left(dt, (double)t, t_end)) { st = ST_DONE_TIME; break; }
+        if (k >= max_steps) { st = ST_DONE_STEPS; break; }
+        const R* xmon;
+        if (integrator == 0) {
+            hermite_step(n, x.data(), v.data(), m.data(), h, n_corr);
+            xmon = x.data();
+        } else {
+            mvs_step(s, m.data(), h);
+            from_dh<R>(s, m.data(), xm.data(), nullptr);
+            xmon = xm.data();
+        }
+        t += h;
+        ++k;
+        const int mon = monitors(n, xmon, r_close, r_eject);
+        if (mon != ST_ACTIVE) { st = mon; break; }
+    }
+    if (integrator == 1) from_dh(s, m.data(), x.data(), v.data());
+    for (int q = 0; q < 3 * n; ++q) { pos[q] = (double)x[q]; vel[q] = (double)v[q]; }
+    *time = (double)t;
+    *status = st;
+    *nsteps += k;
+}
+
+}  // namespace
+
+// ===================================================================================================
+// C interface (ctypes).  prec: 0 = double, 1 = long double.  All return 0 on success, -1 on bad arguments.
+// ===================================================================================================
+extern "C" {
+
+int orc_acc_jerk(int n, const double* x, const double* v, const double* m, double* a, double* j, int prec) {
+    if (n < 2 || !x || !v || !m || !a || !j) return -1;
+    if (prec == 0) {
+        eval_acc_jerk<double>(n, x, v, m, a, j);
+    } else {
+        std::vector<long double> X(x, x + 3 * n), V(v, v + 3 * n), M(m, m + n), A(3 * n), J(3 * n);
+        eval_acc_jerk<long double>(n, X.data(), V.data(), M.data(), A.data(), J.data());
+        for (int q = 0; q < 3 * n; ++q) { a[q] = (double)A[q]; j[q] = (double)J[q]; }
+    }
+    return 0;
+}
+
+// n_corr corrector iterations (the method uses 2; other values exist only for the R5b identity test)
+int orc_hermite_step(int n, double* x, double* v, const double* m, double h, int n_corr, int prec) {
+    if (n < 2 || !x || !v || !m) return -1;
+    if (prec == 0) {
+        hermite_step<double>(n, x, v, m, h, n_corr);
+    } else {
+        std::vector<long double> X(x, x + 3 * n), V(v, v + 3 * n), M(m, m + n);
+        hermite_step<long double>(n, X.data(), V.data(), M.data(), (long double)h, n_corr);
+        for (int q = 0; q < 3 * n; ++q) { x[q] = (double)X[q]; v[q] = (double)V[q]; }
+    }
+    return 0;
+}
+
+// integrator: 0 = Hermite, 1 = MVS.  status/nsteps/time are in-out ([n_sys]); status STOP_* is sticky.
+int orc_integrate(int integrator, int64_t n_sys, int n, double* pos, double* vel, const double* mass, double* time,
+                  int32_t* status, int64_t* nsteps, double dt, double t_end, int64_t max_steps, double r_close,
+                  double r_eject, int prec, int nthreads) {
+    if (n_sys < 0 || n < 2 || !pos || !vel || !mass || !time || !status || !nsteps) return -1;
+    if (!(dt != 0) || !std::isfinite(dt) || max_steps < 0 || (integrator != 0 && integrator != 1)) return -1;
+    if (nthreads < 1) nthreads = 1;
+#pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads)
+    for (int64_t s = 0; s < n_sys; ++s) {
+        double* p = pos + s * 3 * n;
+        double* w = vel + s * 3 * n;
+        const double* mm = mass + s * n;
+        if (prec == 0)
+            run_system<double>(integrator, n, p, w, mm, time + s, status + s, nsteps + s, dt, t_end, max_steps, r_close, r_eject, 2);
+        else
+            run_system<long double>(integrator, n, p, w, mm, time + s, status + s, nsteps + s, dt, t_end, max_steps, r_close, r_eject, 2);
+    }
+    return 0;
+}
+
+int orc_energy(int64_t n_sys, int n, const double* pos, const double* vel, const double* mass, double* E, double* L, int prec) {
+    if (n_sys < 0 || n < 1 || !pos || !vel || !mass || !E) return -1;
+    for (int64_t s = 0; s < n_sys; ++s) {
+        if (prec == 0) {
+            energy_L<double>(n, pos + s * 3 * n, vel + s * 3 * n, mass + s * n, E + s, L ? L + 3 * s : nullptr);
+        } else {
+            std::vector<long double> X(pos + s * 3 * n, pos + (s + 1) * 3 * n), V(vel + s * 3 * n, vel + (s + 1) * 3 * n),
+                M(mass + s * n, mass + (s + 1) * n);
+            long double e, l[3];
+            energy_L<long double>(n, X.data(), V.data(), M.data(), &e, l);
+            E[s] = (double)e;
+            if (L) for (int c = 0; c < 3; ++c) L[3 * s + c] = (double)l[c];
+        }
+    }
+    return 0;
+}
+
+int orc_stumpff(double z, double* c, int prec) {
+    if (!c) return -1;
+    if (prec == 0) {
+        stumpff<double>(z, c);
+    } else {
+        long double C[4];
+        stumpff<long double>((long double)z, C);
+        for (int q = 0; q < 4; ++q) c[q] = (double)C[q];
+    }
+    return 0;
+}
+
+// q, p: [3] in-out.  *iters receives the Newton iteration count (negative: bisection fallback used).
+int orc_kepler_drift(double* q, double* p, double mu, double tau, int prec, int* iters) {
+    if (!q || !p) return -1;
+    int it;
+    if (prec == 0) {
+        it = kepler_drift<double>(q, p, mu, tau);
+    } else {
+        long double Q[3] = {q[0], q[1], q[2]}, P[3] = {p[0], p[1], p[2]};
+        it = kepler_drift<long double>(Q, P, (long double)mu, (long double)tau);
+        for (int c = 0; c < 3; ++c) { q[c] = (double)Q[c]; p[c] = (double)P[c]; }
+    }
+    if (iters) *iters = it;
+    return 0;
+}
+
+// inertial Cartesian -> democratic heliocentric -> inertial Cartesian (for the coordinate round-trip test);
+// Q, V out: [n][3] with row 0 = X_cm / V_cm.
+int orc_dh_roundtrip(int n, const double* x, const double* v, const double* m, double* Q, double* V, double* x2, double* v2) {
+    if (n < 2) return -1;
+    DH<double> s;
+    to_dh<double>(n, x, v, m, s);
+    for (int c = 0; c < 3; ++c) { Q[c] = s.Xcm[c]; V[c] = s.Vcm[c]; }
+    for (int q = 3; q < 3 * n; ++q) { Q[q] = s.Q[q]; V[q] = s.V[q]; }
+    from_dh<double>(s, m, x2, v2);
+    return 0;
+}
+
+}  // extern "C"

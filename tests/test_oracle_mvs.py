@@ -1,0 +1,202 @@
+"""Pins for the MVS half of the CPU oracle: Stumpff closed forms, exact Kepler flow (Kepler's equation solved
+independently), orbit invariants for hyperbolic motion, test-particle exactness of the whole step, 2nd-order
+convergence to the Hermite oracle, exact conservation of L and linear momentum, bounded energy error, reversal.
+`P:L<n>` = /root/reference/PAPER.md line n; R-M<k> = DESIGN.md §3 readings.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1208_1157_b200 import workloads as W
+
+
+# ------------------------------------------------------------------------------------------ Stumpff
+@pytest.mark.parametrize("z", [1.0, 2.5, 9.0, 40.0, 157.0])
+def test_stumpff_positive_argument_closed_forms(z):
+    s = math.sqrt(z)
+    c = oracle.stumpff(z)
+    ref = [math.cos(s), math.sin(s) / s, (1 - math.cos(s)) / z, (s - math.sin(s)) / (z * s)]
+    np.testing.assert_allclose(c, ref, rtol=0, atol=3e-14)
+
+
+@pytest.mark.parametrize("z", [-0.7, -3.0, -25.0])
+def test_stumpff_negative_argument_closed_forms(z):
+    s = math.sqrt(-z)
+    c = oracle.stumpff(z)
+    ref = [math.cosh(s), math.sinh(s) / s, (math.cosh(s) - 1) / (-z), (math.sinh(s) - s) / (-z * s)]
+    np.testing.assert_allclose(c, ref, rtol=2e-14)
+
+
+def test_stumpff_small_argument_and_recurrences():
+    assert np.allclose(oracle.stumpff(0.0), [1.0, 1.0, 0.5, 1.0 / 6.0], rtol=0, atol=0)
+    for z in (1e-8, -1e-5, 3e-3, 0.099, 0.101, -0.4, 0.4):
+        c = oracle.stumpff(z)
+        cl = oracle.stumpff(z, prec=oracle.LONG_DOUBLE)
+        np.testing.assert_allclose(c, cl, rtol=4e-16)
+        # c_n(z) = 1/n! - z c_{n+2}(z)
+        assert abs(c[0] - (1 - z * c[2])) < 3e-16 and abs(c[1] - (1 - z * c[3])) < 3e-16
+        # first two series terms, pinned by hand: c2 = 1/2 - z/24 + z^2/720, c3 = 1/6 - z/120 + z^2/5040
+        assert abs(c[2] - (0.5 - z / 24 + z * z / 720)) < abs(z) ** 3 / 40320 * 1.01 + 1e-16
+        assert abs(c[3] - (1 / 6 - z / 120 + z * z / 5040)) < abs(z) ** 3 / 362880 * 1.01 + 1e-16
+
+
+# ------------------------------------------------------------------------------------------ Kepler drift
+def _kepler_state(a, e, M, mu, inc=0.3, Om=1.0, om=2.0):
+    f = lambda s: np.array([s])
+    q, p = W.elements_to_cartesian(f(a), f(e), f(inc), f(Om), f(om), f(M), mu)
+    return q[0], p[0]
+
+
+@pytest.mark.parametrize("e", [0.0, 0.05, 0.5, 0.85])
+@pytest.mark.parametrize("tau", [0.05, 1.3, 7.0, -2.2, 25.0])
+def test_kepler_drift_matches_keplers_equation(e, tau):
+    # "advanced exactly along a Keplerian orbit for an arbitrary dt simply by increasing the mean anomaly"
+    a, mu, M0 = 1.3, 1.0, 0.7
+    q0, p0 = _kepler_state(a, e, M0, mu)
+    q1, p1, it = oracle.kepler_drift(q0, p0, mu, tau)
+    qe, pe = _kepler_state(a, e, M0 + math.sqrt(mu / a**3) * tau, mu)
+    np.testing.assert_allclose(q1, qe, rtol=0, atol=3e-14 * (1 + abs(tau)))
+    np.testing.assert_allclose(p1, pe, rtol=0, atol=3e-14 * (1 + abs(tau)) / (1 - e))
+
+
+def test_kepler_drift_seven_steps_per_period_returns_to_start():
+    # App. B: test particle, e = 0.5, 7 steps per period -> 4.7e-15
+    a, e, mu = 1.0, 0.5, 1.0
+    q0, p0 = _kepler_state(a, e, 0.3, mu)
+    q, p = q0, p0
+    for _ in range(7):
+        q, p, it = oracle.kepler_drift(q, p, mu, 2 * math.pi / 7)
+        assert 0 < it < 12
+    assert np.abs(q - q0).max() < 5e-14 and np.abs(p - p0).max() < 5e-14
+
+
+def test_kepler_drift_hyperbolic_conserves_orbit_invariants():
+    mu = 1.0
+    q0 = np.array([1.0, 0.2, -0.1])
+    p0 = np.array([0.3, 1.9, 0.4])  # v^2 = 3.86 > 2 mu / r: unbound
+    assert p0 @ p0 > 2 * mu / np.linalg.norm(q0)
+
+    def invariants(q, p):
+        r = np.linalg.norm(q)
+        h = np.cross(q, p)
+        return p @ p / 2 - mu / r, h, np.cross(p, h) / mu - q / r
+
+    E0, h0, e0 = invariants(q0, p0)
+    q1, p1, _ = oracle.kepler_drift(q0, p0, mu, 3.0)
+    E1, h1, e1 = invariants(q1, p1)
+    assert abs(E1 - E0) < 1e-14 and np.abs(h1 - h0).max() < 1e-14 and np.abs(e1 - e0).max() < 1e-14
+    # group property: drift(3) = drift(1.2) then drift(1.8); and drift(-3) inverts it
+    qa, pa, _ = oracle.kepler_drift(q0, p0, mu, 1.2)
+    qb, pb, _ = oracle.kepler_drift(qa, pa, mu, 1.8)
+    assert np.abs(qb - q1).max() < 1e-13 and np.abs(pb - p1).max() < 1e-13
+    qc, pc, _ = oracle.kepler_drift(q1, p1, mu, -3.0)
+    assert np.abs(qc - q0).max() < 1e-13 and np.abs(pc - p0).max() < 1e-13
+
+
+def test_kepler_drift_long_double_agrees():
+    q0, p0 = _kepler_state(0.7, 0.3, 2.0, 1.0)
+    q1, p1, _ = oracle.kepler_drift(q0, p0, 1.0, 0.05)
+    q2, p2, _ = oracle.kepler_drift(q0, p0, 1.0, 0.05, prec=oracle.LONG_DOUBLE)
+    assert np.abs(q1 - q2).max() < 5e-16 and np.abs(p1 - p2).max() < 1e-15
+
+
+# ------------------------------------------------------------------------------------------ coordinates
+def test_democratic_heliocentric_round_trip():
+    pos, vel, mass = W.generate(4, n_sys=2)
+    for s in range(2):
+        Q, V, x2, v2 = oracle.dh_roundtrip(pos[s], vel[s], mass[s])
+        np.testing.assert_allclose(x2, pos[s], rtol=0, atol=5e-16)
+        np.testing.assert_allclose(v2, vel[s], rtol=0, atol=5e-16)
+        np.testing.assert_allclose(Q[1:], pos[s, 1:] - pos[s, 0], rtol=0, atol=1e-16)   # heliocentric positions
+        np.testing.assert_allclose(Q[0], 0.0, atol=1e-16)                                # barycentric input
+        # barycentric momenta sum to minus the star's
+        Pstar = mass[s, 0] * (vel[s, 0] - V[0])
+        np.testing.assert_allclose((mass[s, 1:, None] * V[1:]).sum(0), -Pstar, rtol=0, atol=1e-18)
+
+
+# ------------------------------------------------------------------------------------------ whole step
+def _mvs(pos, vel, mass, dt, steps, **kw):
+    return oracle.integrate(oracle.MVS, pos, vel, mass, dt=dt, max_steps=steps, **kw)
+
+
+def test_mvs_test_particles_follow_exact_kepler_orbits_for_any_step():
+    # "no mutual planetary perturbations -> arbitrarily long time-step, machine precision"; true in the
+    # test-particle limit (R-M5).  Star at rest at the origin, two massless planets, 3 huge steps.
+    a, e, M0 = np.array([1.0, 2.2]), np.array([0.4, 0.1]), np.array([0.5, 4.0])
+    z = np.zeros(2)
+    q, p = W.elements_to_cartesian(a, e, z + 0.2, z + 0.4, z + 1.0, M0, 1.0)
+    pos = np.concatenate([np.zeros((1, 3)), q])[None]
+    vel = np.concatenate([np.zeros((1, 3)), p])[None]
+    mass = np.array([[1.0, 0.0, 0.0]])
+    dt, steps = 1.7, 3
+    r = _mvs(pos, vel, mass, dt, steps)
+    qe, pe = W.elements_to_cartesian(a, e, z + 0.2, z + 0.4, z + 1.0, M0 + a**-1.5 * dt * steps, 1.0)
+    np.testing.assert_allclose(r["pos"][0, 1:], qe, rtol=0, atol=2e-14)
+    np.testing.assert_allclose(r["vel"][0, 1:], pe, rtol=0, atol=2e-14)
+    np.testing.assert_allclose(r["pos"][0, 0], 0.0, atol=1e-18)
+    assert r["status"][0] == oracle.DONE_STEPS and abs(r["time"][0] - dt * steps) < 1e-15
+
+
+def test_mvs_converges_to_hermite_at_second_order():
+    # R-M1/R-M2: democratic-heliocentric splitting with mu = G m0.  App. B: T = 5, N = 250..2000 ->
+    # 5.95e-8, 1.49e-8, 3.72e-9, 9.30e-10 (ratios 4.000).  With mu = G(m0+m_i) the error stalls near 1e-2.
+    pos, vel, mass = W.generate(4, n_sys=4)
+    T = 5.0
+    ref = oracle.integrate(oracle.HERMITE, pos, vel, mass, dt=T / 20000, max_steps=20000, prec=oracle.LONG_DOUBLE)
+    errs = []
+    for N in (250, 500, 1000, 2000):
+        r = _mvs(pos, vel, mass, T / N, N)
+        errs.append(np.abs(r["pos"] - ref["pos"]).max(axis=(1, 2)))
+    errs = np.array(errs)
+    assert (errs[0] < 5e-5).all() and (errs[0] > 1e-10).all(), errs
+    ratios = errs[:-1] / errs[1:]
+    assert (np.abs(ratios - 4.0) < 0.15).all(), ratios
+
+
+def test_mvs_invariants_and_bounded_energy_error():
+    pos, vel, mass = W.generate(4, n_sys=16)
+    E0, L0 = oracle.energy(pos, vel, mass)
+    r1 = _mvs(pos, vel, mass, 0.05, 1000)
+    r2 = _mvs(pos, vel, mass, 0.05, 4000)
+    for r in (r1, r2):
+        E, L = oracle.energy(r["pos"], r["vel"], mass)
+        # every sub-step conserves total L and total linear momentum exactly (R-M6)
+        assert (np.abs(L - L0).max(axis=1) / np.linalg.norm(L0, axis=1)).max() < 2e-13
+        assert np.abs((mass[:, :, None] * r["vel"]).sum(1)).max() < 1e-17
+        # centre of mass stays at the origin
+        assert np.abs((mass[:, :, None] * r["pos"]).sum(1)).max() < 1e-14
+        assert np.abs(E / E0 - 1).max() < 5e-6  # App. B: median 2e-8, max 1.3e-6, no growth
+    e1 = np.abs(oracle.energy(r1["pos"], r1["vel"], mass)[0] / E0 - 1)
+    e2 = np.abs(oracle.energy(r2["pos"], r2["vel"], mass)[0] / E0 - 1)
+    assert np.median(e2) < 20 * np.median(e1) + 1e-9   # bounded, not secular
+
+
+def test_mvs_reversal():
+    pos, vel, mass = W.generate(4, n_sys=4)
+    f = _mvs(pos, vel, mass, 0.05, 2000)
+    b = oracle.integrate(oracle.MVS, f["pos"], f["vel"], mass, f["time"], dt=-0.05, t_end=-np.inf, max_steps=2000)
+    assert np.abs(b["pos"] - pos).max() < 2e-10 and np.abs(b["vel"] - vel).max() < 2e-10
+    assert np.abs(b["time"]).max() < 1e-10
+
+
+def test_mvs_double_vs_long_double_noise_floor_1000_steps():
+    # R-noise: at 10^3 steps the floor is ~1e-12 (pos) / 2.6e-12 (vel), so 1e-10 is a meaningful parity bar there
+    pos, vel, mass = W.generate(4, n_sys=64)
+    a = _mvs(pos, vel, mass, 0.05, 1000)
+    b = _mvs(pos, vel, mass, 0.05, 1000, prec=oracle.LONG_DOUBLE)
+    sx = np.linalg.norm(b["pos"], axis=2).max(axis=1)
+    sv = np.linalg.norm(b["vel"], axis=2).max(axis=1)
+    assert (np.abs(a["pos"] - b["pos"]).max(axis=(1, 2)) / sx).max() < 2e-11
+    assert (np.abs(a["vel"] - b["vel"]).max(axis=(1, 2)) / sv).max() < 2e-11
+
+
+def test_mvs_monitors_and_time_stop():
+    pos, vel, mass = W.generate(4, n_sys=4)
+    r = _mvs(pos, vel, mass, 0.05, 100, t_end=0.42)
+    assert (r["status"] == oracle.DONE_TIME).all() and (r["nsteps"] == 9).all()
+    # ejection threshold inside the outermost orbit fires on the first step
+    rad = np.linalg.norm(pos, axis=2).max(axis=1)
+    r = _mvs(pos, vel, mass, 0.05, 100, r_eject=float(rad.min()) * 0.5)
+    assert (r["status"] == oracle.STOP_EJECT).all() and (r["nsteps"] == 1).all()
