@@ -1,0 +1,124 @@
+/* ens.h — C ABI of libens: an ensemble of independent few-body systems advanced on one B200 (sm_100a) in FP64.
+ *
+ * The library is the data-parallel hot path of Swarm-NG (arxiv 1208.1157; `P:L<n>` = PAPER.md line n):
+ * the fixed-step 4th-order time-symmetrized Hermite integrator (Alg. 2; Eq. 3-4) and a
+ * mixed-variable symplectic kick / Kepler-drift step, both inside the generic
+ * integrator loop of Alg. 1 with fused stop monitors.  Readings of the garbled or
+ * silent passages (R1..R15, R-M1..R-M7) are listed in DESIGN.md §3.
+ *
+ * Conventions
+ *   - Every function returns an int: 0 = ENS_OK, < 0 = error.  No exception crosses this boundary.
+ *   - Caller arrays are plain C-order FP64:  pos, vel [n_sys][n_body][3];  mass [n_sys][n_body];
+ *     time, E [n_sys];  L [n_sys][3];  status int32 [n_sys];  nsteps int64 [n_sys].
+ *     `memspace` says whether those pointers are HOST (pageable or pinned) or DEVICE (cudaMalloc'd, or the
+ *     data_ptr of a torch CUDA tensor) addresses.  The caller owns them and keeps them alive until the
+ *     call's work on `stream` has run.
+ *   - The handle owns its internal structure-of-arrays device buffers (layout: DESIGN.md §5).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-space calls only
+ *     enqueue work and return.  Host-space calls enqueue the copies on `stream` and then wait for it, so the
+ *     host buffers are complete (get) or reusable (set) on return.
+ *   - Body 0 is the central body.  G = 1.  No softening.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns ENS_ECUDA.
+ */
+#ifndef ENS_H
+#define ENS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define ENS_API __attribute__((visibility("default")))
+#else
+#define ENS_API
+#endif
+
+typedef struct ens ens_t; /* opaque */
+
+enum { ENS_OK = 0, ENS_EINVAL = -1, ENS_ENOMEM = -2, ENS_ECUDA = -3, ENS_ESTATE = -4, ENS_EUNSUPPORTED = -5 };
+enum { ENS_HERMITE = 0, ENS_MVS = 1 };
+enum { ENS_HOST = 0, ENS_DEVICE = 1 };
+/* per-system status (Alg. 1 "state").  DONE_* become ACTIVE again at the next ens_integrate;
+ * STOP_* are sticky until ens_set_state. */
+enum {
+    ENS_ACTIVE = 0,
+    ENS_DONE_TIME = 1,      /* t reached t_end (reading R10: stop when t >= t_end, last step not clipped) */
+    ENS_DONE_STEPS = 2,     /* max_steps taken in this call (Alg. 1 max-iterations) */
+    ENS_STOP_CLOSE = 3,     /* some pair separation < r_close after a step (monitor; R11) */
+    ENS_STOP_EJECT = 4,     /* some body farther than r_eject from the coordinate origin after a step (R11) */
+    ENS_STOP_NONFINITE = 5  /* a position became non-finite */
+};
+
+/* Create an ensemble of n_sys >= 1 systems of 2 <= n_body <= 16 bodies on the current CUDA device and
+ * allocate its device buffers.  *out receives the handle.  EINVAL: bad sizes or out == NULL.
+ * ENOMEM: allocation failed.  ECUDA: no device / CUDA error. */
+ENS_API int ens_create(int64_t n_sys, int n_body, ens_t **out);
+
+/* Free the handle and its buffers (synchronises the device first).  NULL is a no-op returning ENS_OK. */
+ENS_API int ens_destroy(ens_t *e);
+
+/* Load the state of every system (Alg. 1 "load initial configuration onto the GPU"; the only
+ * bulk host->device transfer).  time == NULL means t = 0 for all.  Resets status to ACTIVE and
+ * nsteps to 0.  Transposes the caller's [sys][body][3] arrays into the internal SoA layout on the device.
+ * EINVAL: NULL e/pos/vel/mass or bad memspace. */
+ENS_API int ens_set_state(ens_t *e, const double *pos, const double *vel, const double *mass, const double *time,
+                  int memspace, void *stream);
+
+/* Stop monitors evaluated after every step on the new state (Alg. 1 execute(M); thresholds from
+ * BASELINE.json).  r_close <= 0 disables the close-approach monitor; r_eject = +inf (or <= 0) disables the
+ * ejection monitor.  Strict inequalities: stop if r < r_close, or |x_i| > r_eject.  Default: both disabled.
+ * EINVAL: NULL handle or NaN. */
+ENS_API int ens_set_monitors(ens_t *e, double r_close, double r_eject);
+
+/* Advance every system independently (Alg. 1), entirely on the device, in ONE kernel launch
+ * with the state resident in registers across all steps:
+ *     while status == ACTIVE && steps_this_call < max_steps && time left:  step(dt); t += dt; ++nsteps; monitors
+ * "time left" is direction aware: dt > 0: t < t_end;  dt < 0: t > t_end.  Use t_end = +inf (dt > 0) or -inf
+ * (dt < 0) for pure step-count control.  integrator: ENS_HERMITE = predictor + 2 corrector iterations with 3
+ * acceleration-and-jerk evaluations per step (Alg. 2; R3-R6); ENS_MVS = democratic-heliocentric
+ * half-drift / half-kick / Kepler drift / half-kick / half-drift (R-M1..R-M7), which needs body 0
+ * to dominate the mass.
+ * EINVAL: NULL handle, unknown integrator, dt == 0 or non-finite, NaN t_end, max_steps < 0.
+ * ESTATE: no state was set.  ECUDA: launch failed. */
+ENS_API int ens_integrate(ens_t *e, int integrator, double dt, double t_end, int64_t max_steps, void *stream);
+
+/* Copy the state out (transposing back to [sys][body][3]).  Any out pointer may be NULL (skipped).
+ * ESTATE: no state was set. */
+ENS_API int ens_get_state(const ens_t *e, double *pos, double *vel, double *time, int32_t *status, int64_t *nsteps,
+                  int memspace, void *stream);
+
+/* Total energy E = sum 1/2 m v^2 - sum_{i<k} m_i m_k / r_ik (Eq. 6, each pair once: R9) and, if
+ * L != NULL, total angular momentum sum m x cross v, per system, computed on the device ("only 1-4 values
+ * per system need to be transferred").  EINVAL: NULL e or E.  ESTATE: no state was set. */
+ENS_API int ens_energy(const ens_t *e, double *E, double *L, int memspace, void *stream);
+
+/* Static description of an error code; for ENS_ECUDA the text of the last CUDA error seen by this thread. */
+ENS_API const char *ens_strerror(int code);
+
+/* ---- measurement helpers (not part of the method; used by bench.py and the tests) -------------------- */
+
+/* Sizes the library chose for this handle: out[0] = padded system count of the SoA rows, out[1] = lanes
+ * per system L, out[2] = bodies per lane B, out[3] = threads per block, out[4] = blocks of the last or next
+ * Hermite launch, out[5] = registers per thread of that kernel, out[6] = resident blocks per SM (occupancy
+ * API), out[7] = number of kernels this handle has launched so far. */
+ENS_API int ens_get_info(const ens_t *e, int64_t out[8]);
+
+/* Time (ms, CUDA events on `stream`) the last ens_integrate kernel took; waits for it to finish.
+ * ESTATE if nothing was launched. */
+ENS_API int ens_last_kernel_ms(const ens_t *e, float *ms);
+
+/* FP64 pipe microbenchmark: every thread of a full-occupancy grid runs `iters` rounds of 8 independent
+ * dependent-DFMA chains.  *lane_fma_per_s receives FP64 lane-FMA/s (CUDA-event timed on `stream`), the
+ * measured denominator of the FP64 roofline (MEASURED_PEAKS.json has no FP64 entry). */
+ENS_API int ens_fp64_peak(int64_t iters, double *lane_fma_per_s, void *stream);
+
+/* Device function test hook: y[i] = the library's FP64 reciprocal square root of x[i] (float rsqrt seed +
+ * FP64 refinement, P:L276 / R14), device pointers, n elements. */
+ENS_API int ens_test_rsqrt(const double *x, double *y, int64_t n, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ENS_H */

@@ -1,0 +1,453 @@
+// ens_api.cu — the C ABI of include/ens.h: handle, SoA buffers, AoS<->SoA transposition, energy, helpers.
+// All arithmetic of the method lives in hermite_kernel.cuh / mvs_kernel.cuh; nothing here calls oracle/ and there is
+// no CPU fallback: without a device every call that needs one returns ENS_ECUDA.
+#include <cfloat>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "ens_internal.cuh"
+
+namespace {
+
+thread_local char g_cuda_err[256] = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t err, const char* what) {
+    snprintf(g_cuda_err, sizeof g_cuda_err, "CUDA error in %s: %s", what, cudaGetErrorString(err));
+    (void)cudaGetLastError();  // clear the sticky-less error state
+    return err == cudaErrorMemoryAllocation ? ENS_ENOMEM : ENS_ECUDA;
+}
+#define CU(call)                                            \
+    do {                                                    \
+        cudaError_t err__ = (call);                         \
+        if (err__ != cudaSuccess) return cuda_fail(err__, #call); \
+    } while (0)
+
+constexpr int TILE = 64;  // systems per transposition tile = padding granule of the SoA rows
+
+// ---------------------------------------------------------------------------------------------------------------
+// AoS [n_sys][K] <-> SoA [K][n_pad] transposition through shared memory, 128-bit global accesses on both sides
+// (north_star item 2).  One block per tile of 64 systems; K = 3 n_body (pos, vel) or n_body (mass).
+// Pure data movement: HBM-bound, 16 bytes of traffic per double.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) pack_kernel(const double* __restrict__ src, double* __restrict__ dst,
+                                                   int64_t n_sys, int64_t n_pad, int K, int vec_ok) {
+    extern __shared__ double tile[];  // [TILE][Kp], Kp odd: conflict-free column reads
+    const int Kp = K | 1;
+    const int64_t sys0 = (int64_t)blockIdx.x * TILE;
+    const int nv = (int)((n_sys - sys0 < TILE) ? (n_sys - sys0) : TILE);
+    const int total = nv * K;
+    const double* s = src + sys0 * K;
+    if (vec_ok && (total & 1) == 0) {
+        const double2* s2 = reinterpret_cast<const double2*>(s);
+        for (int i = threadIdx.x; i < total / 2; i += blockDim.x) {
+            const double2 w = s2[i];
+            const int i0 = 2 * i, i1 = 2 * i + 1;
+            tile[(i0 / K) * Kp + (i0 % K)] = w.x;
+            tile[(i1 / K) * Kp + (i1 % K)] = w.y;
+        }
+    } else {
+        for (int i = threadIdx.x; i < total; i += blockDim.x) tile[(i / K) * Kp + (i % K)] = s[i];
+    }
+    __syncthreads();
+    // rows of the SoA: two consecutive systems per thread (sys0 and n_pad are multiples of 64: 16-byte aligned)
+    for (int i = threadIdx.x; i < K * (TILE / 2); i += blockDim.x) {
+        const int k = i / (TILE / 2), sp = (i % (TILE / 2)) * 2;
+        double2 w;
+        w.x = sp < nv ? tile[sp * Kp + k] : 0.0;
+        w.y = sp + 1 < nv ? tile[(sp + 1) * Kp + k] : 0.0;
+        *reinterpret_cast<double2*>(dst + (int64_t)k * n_pad + sys0 + sp) = w;
+    }
+}
+
+__global__ void __launch_bounds__(256) unpack_kernel(const double* __restrict__ src, double* __restrict__ dst,
+                                                     int64_t n_sys, int64_t n_pad, int K, int vec_ok) {
+    extern __shared__ double tile[];
+    const int Kp = K | 1;
+    const int64_t sys0 = (int64_t)blockIdx.x * TILE;
+    const int nv = (int)((n_sys - sys0 < TILE) ? (n_sys - sys0) : TILE);
+    for (int i = threadIdx.x; i < K * (TILE / 2); i += blockDim.x) {
+        const int k = i / (TILE / 2), sp = (i % (TILE / 2)) * 2;
+        const double2 w = *reinterpret_cast<const double2*>(src + (int64_t)k * n_pad + sys0 + sp);
+        tile[sp * Kp + k] = w.x;
+        tile[(sp + 1) * Kp + k] = w.y;
+    }
+    __syncthreads();
+    const int total = nv * K;
+    double* d = dst + sys0 * K;
+    if (vec_ok && (total & 1) == 0) {
+        double2* d2 = reinterpret_cast<double2*>(d);
+        for (int i = threadIdx.x; i < total / 2; i += blockDim.x) {
+            const int i0 = 2 * i, i1 = 2 * i + 1;
+            double2 w;
+            w.x = tile[(i0 / K) * Kp + (i0 % K)];
+            w.y = tile[(i1 / K) * Kp + (i1 % K)];
+            d2[i] = w;
+        }
+    } else {
+        for (int i = threadIdx.x; i < total; i += blockDim.x) d[i] = tile[(i / K) * Kp + (i % K)];
+    }
+}
+
+__global__ void reset_kernel(double* time, int32_t* status, int64_t* nsteps, const double* time_src, int64_t n_sys,
+                             int64_t n_pad) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_pad) return;
+    time[i] = (i < n_sys && time_src) ? time_src[i] : 0.0;
+    status[i] = ENS_ACTIVE;
+    nsteps[i] = 0;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Energy and angular momentum, Eq. 6 with each unordered pair once (R9).  One thread per system reading
+// the SoA rows (coalesced); correctly rounded sqrt and divide.  HBM-bound: (7 n_body + 4) * 8 bytes per system.
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) energy_kernel(ensd::View e, double* __restrict__ E, double* __restrict__ Lout) {
+    const int64_t sys = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (sys >= e.n_sys) return;
+    const int n = e.n_body;
+    double x[16][3], m[16];
+    double ke = 0.0, pe = 0.0, L[3] = {0.0, 0.0, 0.0};
+    for (int i = 0; i < n; ++i) {
+        double v[3];
+        for (int c = 0; c < 3; ++c) {
+            x[i][c] = e.pos[(int64_t)(i * 3 + c) * e.n_pad + sys];
+            v[c] = e.vel[(int64_t)(i * 3 + c) * e.n_pad + sys];
+        }
+        m[i] = e.mass[(int64_t)i * e.n_pad + sys];
+        ke += 0.5 * m[i] * (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+        L[0] += m[i] * (x[i][1] * v[2] - x[i][2] * v[1]);
+        L[1] += m[i] * (x[i][2] * v[0] - x[i][0] * v[2]);
+        L[2] += m[i] * (x[i][0] * v[1] - x[i][1] * v[0]);
+    }
+    for (int i = 0; i < n; ++i)
+        for (int k = i + 1; k < n; ++k) {
+            const double dx = x[k][0] - x[i][0], dy = x[k][1] - x[i][1], dz = x[k][2] - x[i][2];
+            pe -= m[i] * m[k] / sqrt(dx * dx + dy * dy + dz * dz);
+        }
+    E[sys] = ke + pe;
+    if (Lout) {
+        Lout[3 * sys + 0] = L[0];
+        Lout[3 * sys + 1] = L[1];
+        Lout[3 * sys + 2] = L[2];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// FP64 pipe microbenchmark: 8 independent DFMA chains per thread (MEASURED_PEAKS.json has no FP64
+// entry, so the denominator of "% of FP64 peak" is measured here).
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dfma_kernel(int64_t iters, double seed, double* out) {
+    double a0 = seed, a1 = seed + 1, a2 = seed + 2, a3 = seed + 3, a4 = seed + 4, a5 = seed + 5, a6 = seed + 6,
+           a7 = seed + 7;
+    const double b = 0.999999, c = 1e-9;
+    for (int64_t i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            a0 = fma(a0, b, c); a1 = fma(a1, b, c); a2 = fma(a2, b, c); a3 = fma(a3, b, c);
+            a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
+        }
+    }
+    const double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+    if (r == 12345.678) out[0] = r;  // never true; keeps the chains alive
+}
+
+
+}  // namespace
+
+struct ens {
+    ensd::View v;
+    double r_close, r_eject;
+    bool have_state;
+    int device;
+    // device staging (AoS) for host-space calls, allocated on first use
+    double* stage;        // [n_sys * n_body * 7] : pos | vel | mass
+    double* stage_small;  // [n_sys * 4] : time / E | L   (also int32 status, int64 nsteps reuse)
+    ensd::KernelInfo hermite, mvs;
+    int threads_override;
+    int64_t last_blocks;
+    const void* last_fn;
+    int64_t launches;
+    cudaEvent_t ev0, ev1;
+    bool timed;
+};
+
+namespace {
+
+int ensure_stage(ens* e) {
+    const int64_t n = e->v.n_sys, nb = e->v.n_body;
+    if (!e->stage) CU(cudaMalloc(&e->stage, sizeof(double) * n * nb * 7));
+    if (!e->stage_small) CU(cudaMalloc(&e->stage_small, sizeof(double) * n * 4));
+    return ENS_OK;
+}
+
+int64_t tiles(const ens* e) { return e->v.n_pad / TILE; }
+size_t tile_smem(int K) { return sizeof(double) * TILE * (size_t)(K | 1); }
+int aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+}  // namespace
+
+extern "C" {
+
+const char* ens_strerror(int code) {
+    switch (code) {
+        case ENS_OK: return "ok";
+        case ENS_EINVAL: return "invalid argument";
+        case ENS_ENOMEM: return "out of device memory";
+        case ENS_ECUDA: return g_cuda_err;
+        case ENS_ESTATE: return "no state set (call ens_set_state first)";
+        case ENS_EUNSUPPORTED: return "unsupported configuration";
+        default: return "unknown error code";
+    }
+}
+
+int ens_create(int64_t n_sys, int n_body, ens_t** out) {
+    if (!out) return ENS_EINVAL;
+    *out = nullptr;
+    if (n_sys < 1 || n_body < 2 || n_body > 16) return ENS_EINVAL;
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    ens* e = new (std::nothrow) ens();
+    if (!e) return ENS_ENOMEM;
+    memset(e, 0, sizeof *e);
+    e->device = dev;
+    e->v.n_sys = n_sys;
+    e->v.n_body = n_body;
+    e->v.n_pad = (n_sys + TILE - 1) / TILE * TILE;
+    e->r_close = 0.0;
+    e->r_eject = INFINITY;
+    const int64_t np = e->v.n_pad;
+    cudaError_t err = cudaSuccess;
+    auto alloc = [&](void** p, size_t bytes) {
+        if (err == cudaSuccess) err = cudaMalloc(p, bytes);
+    };
+    alloc((void**)&e->v.pos, sizeof(double) * np * n_body * 3);
+    alloc((void**)&e->v.vel, sizeof(double) * np * n_body * 3);
+    alloc((void**)&e->v.mass, sizeof(double) * np * n_body);
+    alloc((void**)&e->v.time, sizeof(double) * np);
+    alloc((void**)&e->v.status, sizeof(int32_t) * np);
+    alloc((void**)&e->v.nsteps, sizeof(int64_t) * np);
+    if (err == cudaSuccess) err = cudaEventCreate(&e->ev0);
+    if (err == cudaSuccess) err = cudaEventCreate(&e->ev1);
+    if (err != cudaSuccess) {
+        const int rc = cuda_fail(err, "ens_create");
+        ens_destroy(e);
+        return rc;
+    }
+    e->hermite = ensd::hermite_kernel_for(n_body);
+    e->mvs = ensd::mvs_kernel_for(n_body);
+    const char* env = getenv("ENS_THREADS");
+    e->threads_override = env ? atoi(env) : 0;
+    if (e->threads_override < 32 || e->threads_override > 1024 || (e->threads_override & 31)) e->threads_override = 0;
+    *out = e;
+    return ENS_OK;
+}
+
+int ens_destroy(ens_t* e) {
+    if (!e) return ENS_OK;
+    cudaDeviceSynchronize();
+    cudaFree(e->v.pos);
+    cudaFree(e->v.vel);
+    cudaFree(e->v.mass);
+    cudaFree(e->v.time);
+    cudaFree(e->v.status);
+    cudaFree(e->v.nsteps);
+    cudaFree(e->stage);
+    cudaFree(e->stage_small);
+    if (e->ev0) cudaEventDestroy(e->ev0);
+    if (e->ev1) cudaEventDestroy(e->ev1);
+    (void)cudaGetLastError();
+    delete e;
+    return ENS_OK;
+}
+
+int ens_set_monitors(ens_t* e, double r_close, double r_eject) {
+    if (!e || std::isnan(r_close) || std::isnan(r_eject)) return ENS_EINVAL;
+    e->r_close = r_close > 0.0 ? r_close : 0.0;
+    e->r_eject = r_eject > 0.0 ? r_eject : INFINITY;
+    return ENS_OK;
+}
+
+int ens_set_state(ens_t* e, const double* pos, const double* vel, const double* mass, const double* time, int memspace,
+                  void* stream) {
+    if (!e || !pos || !vel || !mass || (memspace != ENS_HOST && memspace != ENS_DEVICE)) return ENS_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int64_t n = e->v.n_sys, nb = e->v.n_body;
+    const double *dpos = pos, *dvel = vel, *dmass = mass, *dtime = time;
+    if (memspace == ENS_HOST) {
+        const int rc = ensure_stage(e);
+        if (rc) return rc;
+        double* st = e->stage;
+        CU(cudaMemcpyAsync(st, pos, sizeof(double) * n * nb * 3, cudaMemcpyHostToDevice, s));
+        CU(cudaMemcpyAsync(st + n * nb * 3, vel, sizeof(double) * n * nb * 3, cudaMemcpyHostToDevice, s));
+        CU(cudaMemcpyAsync(st + n * nb * 6, mass, sizeof(double) * n * nb, cudaMemcpyHostToDevice, s));
+        dpos = st;
+        dvel = st + n * nb * 3;
+        dmass = st + n * nb * 6;
+        if (time) {
+            CU(cudaMemcpyAsync(e->stage_small, time, sizeof(double) * n, cudaMemcpyHostToDevice, s));
+            dtime = e->stage_small;
+        }
+    }
+    const int K3 = (int)nb * 3, K1 = (int)nb;
+    const unsigned g = (unsigned)tiles(e);
+    pack_kernel<<<g, 256, tile_smem(K3), s>>>(dpos, e->v.pos, n, e->v.n_pad, K3, aligned16(dpos));
+    pack_kernel<<<g, 256, tile_smem(K3), s>>>(dvel, e->v.vel, n, e->v.n_pad, K3, aligned16(dvel));
+    pack_kernel<<<g, 256, tile_smem(K1), s>>>(dmass, e->v.mass, n, e->v.n_pad, K1, aligned16(dmass));
+    reset_kernel<<<(unsigned)((e->v.n_pad + 255) / 256), 256, 0, s>>>(e->v.time, e->v.status, e->v.nsteps, dtime, n,
+                                                                      e->v.n_pad);
+    e->launches += 4;
+    CU(cudaGetLastError());
+    if (memspace == ENS_HOST) CU(cudaStreamSynchronize(s));
+    e->have_state = true;
+    return ENS_OK;
+}
+
+int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max_steps, void* stream) {
+    if (!e || (integrator != ENS_HERMITE && integrator != ENS_MVS)) return ENS_EINVAL;
+    if (!(dt != 0.0) || !std::isfinite(dt) || std::isnan(t_end) || max_steps < 0) return ENS_EINVAL;
+    if (!e->have_state) return ENS_ESTATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    ensd::StepArgs a;
+    a.dt = dt;
+    a.t_end = t_end;
+    a.max_steps = max_steps;
+    const double rc2 = e->r_close * e->r_close;
+    double re2 = e->r_eject * e->r_eject;
+    if (!(re2 < DBL_MAX)) re2 = DBL_MAX;
+    memcpy(&a.rc2_bits, &rc2, 8);
+    memcpy(&a.re2_bits, &re2, 8);
+    const ensd::KernelInfo& ki = integrator == ENS_HERMITE ? e->hermite : e->mvs;
+    if (!ki.fn) return ENS_EUNSUPPORTED;
+    const int threads = e->threads_override ? e->threads_override : ki.threads;
+    CU(cudaEventRecord(e->ev0, s));
+    cudaError_t err = integrator == ENS_HERMITE ? ensd::launch_hermite(e->v, a, threads, s, &e->last_blocks)
+                                                : ensd::launch_mvs(e->v, a, threads, s, &e->last_blocks);
+    if (err != cudaSuccess) return cuda_fail(err, "ens_integrate launch");
+    CU(cudaEventRecord(e->ev1, s));
+    e->last_fn = ki.fn;
+    e->launches += 1;
+    e->timed = true;
+    return ENS_OK;
+}
+
+int ens_get_state(const ens_t* e, double* pos, double* vel, double* time, int32_t* status, int64_t* nsteps,
+                  int memspace, void* stream) {
+    if (!e || (memspace != ENS_HOST && memspace != ENS_DEVICE)) return ENS_EINVAL;
+    if (!e->have_state) return ENS_ESTATE;
+    ens* me = const_cast<ens*>(e);
+    cudaStream_t s = (cudaStream_t)stream;
+    const int64_t n = e->v.n_sys, nb = e->v.n_body;
+    const int K3 = (int)nb * 3;
+    const unsigned g = (unsigned)tiles(e);
+    const cudaMemcpyKind kind = memspace == ENS_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+    if (memspace == ENS_HOST && (pos || vel)) {
+        const int rc = ensure_stage(me);
+        if (rc) return rc;
+    }
+    if (pos) {
+        double* d = memspace == ENS_HOST ? e->stage : pos;
+        unpack_kernel<<<g, 256, tile_smem(K3), s>>>(e->v.pos, d, n, e->v.n_pad, K3, aligned16(d));
+        me->launches += 1;
+        if (memspace == ENS_HOST) CU(cudaMemcpyAsync(pos, d, sizeof(double) * n * nb * 3, kind, s));
+    }
+    if (vel) {
+        double* d = memspace == ENS_HOST ? e->stage + n * nb * 3 : vel;
+        unpack_kernel<<<g, 256, tile_smem(K3), s>>>(e->v.vel, d, n, e->v.n_pad, K3, aligned16(d));
+        me->launches += 1;
+        if (memspace == ENS_HOST) CU(cudaMemcpyAsync(vel, d, sizeof(double) * n * nb * 3, kind, s));
+    }
+    if (time) CU(cudaMemcpyAsync(time, e->v.time, sizeof(double) * n, kind, s));
+    if (status) CU(cudaMemcpyAsync(status, e->v.status, sizeof(int32_t) * n, kind, s));
+    if (nsteps) CU(cudaMemcpyAsync(nsteps, e->v.nsteps, sizeof(int64_t) * n, kind, s));
+    CU(cudaGetLastError());
+    if (memspace == ENS_HOST) CU(cudaStreamSynchronize(s));
+    return ENS_OK;
+}
+
+int ens_energy(const ens_t* e, double* E, double* L, int memspace, void* stream) {
+    if (!e || !E || (memspace != ENS_HOST && memspace != ENS_DEVICE)) return ENS_EINVAL;
+    if (!e->have_state) return ENS_ESTATE;
+    ens* me = const_cast<ens*>(e);
+    cudaStream_t s = (cudaStream_t)stream;
+    const int64_t n = e->v.n_sys;
+    double *dE = E, *dL = L;
+    if (memspace == ENS_HOST) {
+        const int rc = ensure_stage(me);
+        if (rc) return rc;
+        dE = e->stage_small;
+        dL = L ? e->stage_small + n : nullptr;
+    }
+    energy_kernel<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(e->v, dE, dL);
+    me->launches += 1;
+    CU(cudaGetLastError());
+    if (memspace == ENS_HOST) {
+        CU(cudaMemcpyAsync(E, dE, sizeof(double) * n, cudaMemcpyDeviceToHost, s));
+        if (L) CU(cudaMemcpyAsync(L, dL, sizeof(double) * n * 3, cudaMemcpyDeviceToHost, s));
+        CU(cudaStreamSynchronize(s));
+    }
+    return ENS_OK;
+}
+
+int ens_get_info(const ens_t* e, int64_t out[8]) {
+    if (!e || !out) return ENS_EINVAL;
+    const ensd::KernelInfo& ki = (e->last_fn && e->last_fn == e->mvs.fn) ? e->mvs : e->hermite;
+    const int threads = e->threads_override ? e->threads_override : ki.threads;
+    out[0] = e->v.n_pad;
+    out[1] = ki.shape.L;
+    out[2] = ki.shape.B;
+    out[3] = threads;
+    const int64_t sys_per_warp = 32 / (ki.shape.L > 0 ? ki.shape.L : 1);
+    const int64_t warps = (e->v.n_sys + sys_per_warp - 1) / sys_per_warp;
+    out[4] = e->last_blocks ? e->last_blocks : (warps + threads / 32 - 1) / (threads / 32);
+    out[5] = out[6] = 0;
+    if (ki.fn) {
+        cudaFuncAttributes fa;
+        CU(cudaFuncGetAttributes(&fa, ki.fn));
+        out[5] = fa.numRegs;
+        int nb = 0;
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, ki.fn, threads, 0));
+        out[6] = nb;
+    }
+    out[7] = e->launches;
+    return ENS_OK;
+}
+
+int ens_last_kernel_ms(const ens_t* e, float* ms) {
+    if (!e || !ms) return ENS_EINVAL;
+    if (!e->timed) return ENS_ESTATE;
+    CU(cudaEventSynchronize(e->ev1));
+    CU(cudaEventElapsedTime(ms, e->ev0, e->ev1));
+    return ENS_OK;
+}
+
+int ens_fp64_peak(int64_t iters, double* lane_fma_per_s, void* stream) {
+    if (iters < 1 || !lane_fma_per_s) return ENS_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double* out = nullptr;
+    CU(cudaMalloc(&out, sizeof(double)));
+    cudaEvent_t a, b;
+    CU(cudaEventCreate(&a));
+    CU(cudaEventCreate(&b));
+    const int blocks = sms * 8, threads = 256;  // 64 warps per SM
+    dfma_kernel<<<blocks, threads, 0, s>>>(iters / 8 + 1, 1.0, out);  // warm-up
+    CU(cudaEventRecord(a, s));
+    dfma_kernel<<<blocks, threads, 0, s>>>(iters, 1.0, out);
+    CU(cudaEventRecord(b, s));
+    CU(cudaEventSynchronize(b));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, a, b));
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    cudaFree(out);
+    CU(cudaGetLastError());
+    *lane_fma_per_s = (double)blocks * threads * (double)iters * 64.0 / (ms * 1e-3);
+    return ENS_OK;
+}
+
+}  // extern "C"

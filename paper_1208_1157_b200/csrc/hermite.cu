@@ -1,0 +1,106 @@
+// hermite.cu — instantiations of the fused Hermite step-loop kernel and the n_body -> (L, B) dispatch.
+#include "hermite_kernel.cuh"
+
+namespace ensd {
+
+namespace {
+
+// n_body -> lanes per system L (odd), bodies per lane B, L * B >= n_body.  Exact fits for 2-6, 9, 10, 12, 15;
+// the others run in the next larger shape with massless dummy slots.
+template <int N> struct ShapeOf;
+#define ENS_SHAPE(N_, L_, B_, UNROLL_, THREADS_, MINB_)                 \
+    template <> struct ShapeOf<N_> {                                    \
+        static constexpr int L = L_, B = B_, THREADS = THREADS_, MINB = MINB_; \
+        static constexpr bool UNROLL = UNROLL_;                         \
+    };
+//        N  L  B  unroll threads minBlocks
+ENS_SHAPE(2, 1, 2, true, 64, 1)
+ENS_SHAPE(3, 1, 3, true, 64, 1)
+ENS_SHAPE(4, 1, 4, false, 64, 1)
+ENS_SHAPE(5, 1, 5, false, 64, 1)
+ENS_SHAPE(6, 3, 2, false, 64, 1)
+ENS_SHAPE(7, 3, 3, false, 64, 1)
+ENS_SHAPE(8, 3, 3, false, 64, 1)
+ENS_SHAPE(9, 3, 3, false, 64, 1)
+ENS_SHAPE(10, 5, 2, false, 64, 1)
+ENS_SHAPE(11, 3, 4, false, 64, 1)
+ENS_SHAPE(12, 3, 4, false, 64, 1)
+ENS_SHAPE(13, 5, 3, false, 64, 1)
+ENS_SHAPE(14, 5, 3, false, 64, 1)
+ENS_SHAPE(15, 5, 3, false, 64, 1)
+ENS_SHAPE(16, 5, 4, false, 64, 1)
+#undef ENS_SHAPE
+
+template <int N>
+constexpr auto kernel_ptr() {
+    using S = ShapeOf<N>;
+    return &hermite_kernel<N, S::L, S::B, S::UNROLL, 128, S::MINB>;
+}
+
+template <int N>
+KernelInfo info_of() {
+    using S = ShapeOf<N>;
+    KernelInfo k;
+    k.fn = (const void*)kernel_ptr<N>();
+    k.shape.L = S::L;
+    k.shape.B = S::B;
+    k.threads = S::THREADS;
+    return k;
+}
+
+template <int N>
+cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
+    using S = ShapeOf<N>;
+    if (threads > 128) threads = 128;  // __launch_bounds__ of the kernel
+    const int64_t sys_per_warp = 32 / S::L;
+    const int64_t warps = (v.n_sys + sys_per_warp - 1) / sys_per_warp;
+    const int wpb = threads / 32;
+    const int64_t blocks = (warps + wpb - 1) / wpb;
+    if (blocks_out) *blocks_out = blocks;
+    kernel_ptr<N>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+#define ENS_FOR_EACH_N(X) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
+
+KernelInfo hermite_kernel_for(int n_body) {
+    switch (n_body) {
+#define X(N_) \
+    case N_: return info_of<N_>();
+        ENS_FOR_EACH_N(X)
+#undef X
+    }
+    KernelInfo none;
+    none.fn = nullptr;
+    none.shape.L = none.shape.B = 0;
+    none.threads = 0;
+    return none;
+}
+
+cudaError_t launch_hermite(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
+    switch (v.n_body) {
+#define X(N_) \
+    case N_: return launch_n<N_>(v, a, threads, s, blocks_out);
+        ENS_FOR_EACH_N(X)
+#undef X
+    }
+    return cudaErrorInvalidValue;
+}
+
+namespace {
+__global__ void rsqrt_test_kernel(const double* x, double* y, int64_t n) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) y[i] = rsqrt_f64(x[i]);
+}
+}  // namespace
+
+}  // namespace ensd
+
+extern "C" ENS_API int ens_test_rsqrt(const double* x, double* y, int64_t n, void* stream) {
+    if (!x || !y || n < 0) return ENS_EINVAL;
+    if (n == 0) return ENS_OK;
+    ensd::rsqrt_test_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(x, y, n);
+    return cudaGetLastError() == cudaSuccess ? ENS_OK : ENS_ECUDA;
+}

@@ -1,0 +1,338 @@
+// hermite_kernel.cuh — the fused Hermite step loop for sm_100a (FP64 CUDA cores; no tensor cores: not a contraction).
+//
+// One launch = Alg. 1 for every system: state is read from the SoA rows once, lives in registers
+// for all steps and is written back once.  One step = Alg. 2: predictor (Eq. 3,
+// P:L79-81), then two corrector iterations (Eq. 4, read as R3-R5 of DESIGN.md §3), each preceded by an
+// acceleration-and-jerk evaluation (Eq. 1; jerk P:L77) — 3 evaluations per step (R6).
+//
+// Work split (differs from the paper's Fermi design): a system is held by L lanes of a warp (L odd),
+// B bodies per lane.  Every unordered pair is evaluated exactly once:
+//   * pairs of two bodies of the same lane: in registers;
+//   * pairs across lanes: ring schedule.  At shift s = 1..(L-1)/2 lane l fetches the bodies of lane (l+s) mod L
+//     with warp shuffles, accumulates its own half of each pair in registers and the visitor's half (Newton's
+//     third law) in a temporary that is shuffled back to the owner.  No shared memory, no __syncthreads.
+// L = 1 (n_body <= 5) is "one system per thread" and contains no shuffle at all.
+//
+// The first evaluation of step k+1 is the evaluation of the post-step-k state, so its minimum pair distance IS
+// the close-approach monitor Alg. 1 places after step k: monitors cost no extra pair work, and a
+// launch costs 3 evaluations per step + 1.  A system that stops (monitor, t_end, step budget) goes inactive;
+// the warp keeps looping only while some lane is active and inactive lanes skip the step body, so finished
+// systems consume no FP64 issue slots (north_star item 3).
+#pragma once
+#include "ens_internal.cuh"
+
+namespace ensd {
+
+typedef unsigned long long u64;
+
+__device__ __forceinline__ u64 dbits(double x) { return (u64)__double_as_longlong(x); }
+
+// FP64 reciprocal square root (P:L276 used the Fermi hardware rsqrt; R14): MUFU.RSQ seed of the value rounded
+// to FP32 (relative error <= 2^-22) and one cubic Newton-Halley step in FP64,
+//   e = 1 - r2 y0^2,  y = y0 + y0 e (1/2 + 3/8 e),   remaining error ~ (5/16) e^3 < 2^-66 plus rounding: <= 1 ulp
+// (tests/test_gpu_device_functions.py measures it).  Valid for r2 inside the FP32 normal range, 1.2e-38 < r2 <
+// 3.4e38, i.e. separations between 1e-19 and 1e19 length units.
+__device__ __forceinline__ double rsqrt_f64(double r2) {
+    float s;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(__double2float_rn(r2)));
+    const double y0 = (double)s;
+    const double t = r2 * y0;
+    const double e = fma(-t, y0, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    const double q = y0 * e;
+    return fma(q, p, y0);
+}
+
+// One unordered pair (i, k): adds m_k f to (a_i, j_i) and -m_i f to (a_k, j_k), with
+//   f_a = dx / r^3,  f_j = (dv - 3 (dx.dv) dx / r^2) / r^3,  dx = x_k - x_i, dv = v_k - v_i   (Eq. 1 and d/dt, R1-R2).
+// 38 FP64 instructions.  r2 is returned for the close-approach monitor.
+__device__ __forceinline__ double pair_acc_jerk(const double (&xi)[3], const double (&vi)[3], double mi,
+                                                double (&ai)[3], double (&ji)[3], const double (&xk)[3],
+                                                const double (&vk)[3], double mk, double (&ak)[3],
+                                                double (&jk)[3]) {
+    double dx[3], dv[3], u[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        dx[c] = xk[c] - xi[c];
+        dv[c] = vk[c] - vi[c];
+    }
+    const double r2 = fma(dx[2], dx[2], fma(dx[1], dx[1], dx[0] * dx[0]));
+    const double rv = fma(dx[2], dv[2], fma(dx[1], dv[1], dx[0] * dv[0]));
+    const double y = rsqrt_f64(r2);
+    const double y2 = y * y;
+    const double y3 = y2 * y;
+    const double s3 = (-3.0 * y2) * rv;
+    const double wi = mk * y3;
+    const double wk = -mi * y3;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        u[c] = fma(s3, dx[c], dv[c]);
+        ai[c] = fma(wi, dx[c], ai[c]);
+        ji[c] = fma(wi, u[c], ji[c]);
+        ak[c] = fma(wk, dx[c], ak[c]);
+        jk[c] = fma(wk, u[c], jk[c]);
+    }
+    return r2;
+}
+
+__device__ __forceinline__ void min_bits(u64& acc, double r2, bool valid = true) {
+    // r2 >= 0 or NaN: unsigned order of the bit patterns is the numeric order and NaN sorts above +inf, so this
+    // minimum runs on the integer ALU, not the FP64 pipe.
+    const u64 b = valid ? dbits(r2) : ~0ull;
+    acc = b < acc ? b : acc;
+}
+
+// Acceleration and jerk of the B bodies this lane owns, every pair of the system once.
+// l = lane index inside the system (0..L-1), base = first lane of the system in the warp, amask = active lanes.
+template <int N, int L, int B>
+__device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const double (&v)[B][3], const double (&m)[B],
+                                              double (&a)[B][3], double (&j)[B][3], u64& r2min, int l, int base,
+                                              unsigned amask) {
+    constexpr bool PADDED = (L * B != N);
+#pragma unroll
+    for (int b = 0; b < B; ++b)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) a[b][c] = j[b][c] = 0.0;
+    r2min = ~0ull;
+
+    // pairs inside the lane.  Order: pairs among bodies 1.. first, pairs with local body 0 last, so that on lane 0
+    // every planet receives the star's (largest) contribution last (for L = 1 this is exactly the
+    // oracle's order: planets ascending, then the star).
+#pragma unroll
+    for (int bb = 1; bb <= B; ++bb) {
+        const int b = (bb == B) ? 0 : bb;
+#pragma unroll
+        for (int c = b + 1; c < B; ++c) {
+            const double r2 = pair_acc_jerk(x[b], v[b], m[b], a[b], j[b], x[c], v[c], m[c], a[c], j[c]);
+            min_bits(r2min, r2, !PADDED || (l * B + c < N));
+        }
+    }
+
+    if constexpr (L > 1) {
+#pragma unroll
+        for (int s = 1; s <= (L - 1) / 2; ++s) {
+            int ls = l + s;
+            if (ls >= L) ls -= L;
+            int lr = l - s;
+            if (lr < 0) lr += L;
+            const int src = base + ls;  // whose bodies visit this lane
+            const int ret = base + lr;  // which lane computed the other half of MY bodies' pairs at this shift
+#pragma unroll
+            for (int c = 0; c < B; ++c) {
+                double xv[3], vv[3], av[3] = {0.0, 0.0, 0.0}, jv[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+                for (int q = 0; q < 3; ++q) {
+                    xv[q] = __shfl_sync(amask, x[c][q], src);
+                    vv[q] = __shfl_sync(amask, v[c][q], src);
+                }
+                const double mv = __shfl_sync(amask, m[c], src);
+                const bool vvalid = !PADDED || (ls * B + c < N);
+#pragma unroll
+                for (int b = 0; b < B; ++b) {
+                    const double r2 = pair_acc_jerk(x[b], v[b], m[b], a[b], j[b], xv, vv, mv, av, jv);
+                    min_bits(r2min, r2, vvalid && (!PADDED || (l * B + b < N)));
+                }
+#pragma unroll
+                for (int q = 0; q < 3; ++q) {
+                    a[c][q] += __shfl_sync(amask, av[q], ret);
+                    j[c][q] += __shfl_sync(amask, jv[q], ret);
+                }
+            }
+        }
+    }
+}
+
+// bits: 1 = close approach, 2 = ejection, 4 = non-finite position; OR-reduced over the lanes of the system.
+template <int N, int L, int B>
+__device__ __forceinline__ int monitor_flags(const double (&x)[B][3], u64 r2min, const StepArgs& p, int l, int base,
+                                             unsigned amask) {
+    constexpr bool PADDED = (L * B != N);
+    int f = (r2min < p.rc2_bits) ? 1 : 0;
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+        const double d2 = fma(x[b][2], x[b][2], fma(x[b][1], x[b][1], x[b][0] * x[b][0]));
+        const u64 db = dbits(d2);
+        if (!PADDED || (l * B + b < N)) {
+            if (db > p.re2_bits) f |= 2;
+            if (db > 0x7FEFFFFFFFFFFFFFull) f |= 4;  // > DBL_MAX: +inf or NaN
+        }
+    }
+    if constexpr (L > 1) {
+        int g = f;
+#pragma unroll
+        for (int i = 1; i < L; ++i) {
+            int li = l + i;
+            if (li >= L) li -= L;
+            g |= __shfl_sync(amask, f, base + li);
+        }
+        f = g;
+    }
+    return f;
+}
+
+// UNROLL = true: the three evaluations of a step are three inlined copies (straight-line step, best for small
+// pair counts); false: one copy of the evaluation inside a 3-phase loop (keeps large-n kernels inside the
+// instruction cache and the live register set at x, v, C_x, C_v, a, j).
+template <int N, int L, int B, bool UNROLL, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p) {
+    constexpr int S = 32 / L;  // systems per warp
+    constexpr bool PADDED = (L * B != N);
+    const int lane = threadIdx.x & 31;
+    const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int sl = lane / L;
+    const int l = lane - sl * L;
+    const int base = sl * L;
+    const int64_t sys = warp * S + sl;
+    const bool live = (sl < S) && (sys < e.n_sys);
+
+    double X[B][3], V[B][3], m[B];
+    double t = 0.0;
+    int st = ENS_STOP_NONFINITE;
+    bool active = false;
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+        // dummy slot (padded shapes only): massless, at rest, far from everything and from each other
+        const int gid = l * B + b;
+        X[b][0] = 1.0e8 * (double)(gid + 1);
+        X[b][1] = X[b][2] = 0.0;
+        V[b][0] = V[b][1] = V[b][2] = 0.0;
+        m[b] = 0.0;
+    }
+    if (live) {
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const int gid = l * B + b;
+            if (!PADDED || gid < N) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    X[b][c] = e.pos[(int64_t)(gid * 3 + c) * e.n_pad + sys];
+                    V[b][c] = e.vel[(int64_t)(gid * 3 + c) * e.n_pad + sys];
+                }
+                m[b] = e.mass[(int64_t)gid * e.n_pad + sys];
+            }
+        }
+        t = e.time[sys];
+        st = e.status[sys];
+        active = st < ENS_STOP_CLOSE;  // STOP_* are sticky; DONE_* run again
+    }
+    const bool writeback = active;
+
+    // Eq. 3 / Eq. 4 with the step-size powers folded in (algebraically the oracle's formulas):
+    //   x_p = x + h v + h^2/2 a0 + h^3/6 j0          v_p = v + h a0 + h^2/2 j0
+    //   C_x = x + h v + 7/20 h^2 a0 + 1/20 h^3 j0    C_v = v + h/2 a0 + 1/12 h^2 j0
+    //   x_c = C_x + 3/20 h^2 a1 - 1/30 h^3 j1        v_c = C_v + h/2 a1 - 1/12 h^2 j1
+    const double h = p.dt;
+    const double h2 = h * h, h3 = h2 * h;
+    const double p_a = 0.5 * h2, p_j = h3 / 6.0;
+    const double cx_a = 0.35 * h2, cx_j = 0.05 * h3, cv_a = 0.5 * h, cv_j = h2 / 12.0;
+    const double kx_a = 0.15 * h2, kx_j = -h3 / 30.0, kv_a = 0.5 * h, kv_j = -h2 / 12.0;
+    const bool fwd = h > 0.0;
+
+    double Cx[B][3], Cv[B][3];
+    double a[B][3], j[B][3];
+    u64 r2min;
+    int64_t k = 0;
+
+    // phase 0 of the loop below; returns with `active` updated.  X, V hold the accepted state.
+    auto accept_and_predict = [&](unsigned amask) {
+        if (k > 0) {  // monitors act on post-step states only (Alg. 1: advance, then execute(M))
+            const int f = monitor_flags<N, L, B>(X, r2min, p, l, base, amask);
+            if (f) {
+                st = (f & 4) ? ENS_STOP_NONFINITE : (f & 1) ? ENS_STOP_CLOSE : ENS_STOP_EJECT;
+                active = false;
+            }
+        }
+        if (active) {
+            if (!(fwd ? (t < p.t_end) : (t > p.t_end))) {
+                st = ENS_DONE_TIME;
+                active = false;
+            } else if (k >= p.max_steps) {
+                st = ENS_DONE_STEPS;
+                active = false;
+            }
+        }
+        if (active) {
+#pragma unroll
+            for (int b = 0; b < B; ++b)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const double tx = fma(h, V[b][c], X[b][c]);
+                    Cx[b][c] = fma(cx_j, j[b][c], fma(cx_a, a[b][c], tx));
+                    Cv[b][c] = fma(cv_j, j[b][c], fma(cv_a, a[b][c], V[b][c]));
+                    X[b][c] = fma(p_j, j[b][c], fma(p_a, a[b][c], tx));
+                    V[b][c] = fma(p_a, j[b][c], fma(h, a[b][c], V[b][c]));
+                }
+        }
+    };
+    auto correct = [&]() {
+#pragma unroll
+        for (int b = 0; b < B; ++b)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                X[b][c] = fma(kx_j, j[b][c], fma(kx_a, a[b][c], Cx[b][c]));
+                V[b][c] = fma(kv_j, j[b][c], fma(kv_a, a[b][c], Cv[b][c]));
+            }
+    };
+
+    if constexpr (UNROLL) {
+        while (true) {
+            const unsigned amask = __ballot_sync(0xffffffffu, active);
+            if (amask == 0) break;
+            if (active) {
+                eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
+                accept_and_predict(amask);
+                if (active) {
+                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
+                    correct();
+                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
+                    correct();
+                    t += h;
+                    ++k;
+                }
+            }
+        }
+    } else {
+        int phase = 0;
+        while (true) {
+            const unsigned amask = __ballot_sync(0xffffffffu, active);
+            if (amask == 0) break;
+            if (active) {
+                eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
+                if (phase == 0) {
+                    accept_and_predict(amask);
+                    phase = 1;
+                } else {
+                    correct();
+                    if (phase == 2) {
+                        t += h;
+                        ++k;
+                        phase = 0;
+                    } else {
+                        phase = 2;
+                    }
+                }
+            }
+        }
+    }
+
+    if (writeback) {
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const int gid = l * B + b;
+            if (!PADDED || gid < N) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    e.pos[(int64_t)(gid * 3 + c) * e.n_pad + sys] = X[b][c];
+                    e.vel[(int64_t)(gid * 3 + c) * e.n_pad + sys] = V[b][c];
+                }
+            }
+        }
+        if (l == 0) {
+            e.time[sys] = t;
+            e.status[sys] = st;
+            e.nsteps[sys] += k;
+        }
+    }
+}
+
+}  // namespace ensd

@@ -1,0 +1,326 @@
+"""GPU parity of the fused Hermite step loop (libens, through the C ABI) against the CPU oracle on the same seeded
+inputs.  Tolerances (BASELINE.json north_star): config 0 max relative position/velocity difference
+<= 1e-10; longer runs <= 1e-6 per system on systems that never stop, |dE/E| within 1e-9 of the oracle's;
+status and step counts exact (R12)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1208_1157_b200 import ens
+from paper_1208_1157_b200 import workloads as W
+from parity import energy_err, rel_diff, run_cuda, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def test_config0_full_parity():
+    c = W.CONFIGS[0]
+    pos, vel, mass = W.generate(0)
+    g = run_cuda(c, pos, vel, mass, want_energy=True)
+    o = run_oracle(c, pos, vel, mass)
+    assert (g["status"] == ens.DONE_STEPS).all() and (o["status"] == oracle.DONE_STEPS).all()
+    assert (g["nsteps"] == c.steps).all()
+    np.testing.assert_allclose(g["time"], o["time"], rtol=0, atol=1e-9)
+    dp, dv = rel_diff(g["pos"], o["pos"]), rel_diff(g["vel"], o["vel"])
+    print(f"cfg0 parity: pos max {dp.max():.3e} median {np.median(dp):.3e}; vel max {dv.max():.3e}")
+    assert dp.max() <= 1e-10 and dv.max() <= 1e-10
+    # energy error agrees with the oracle's
+    Eo0, _ = oracle.energy(pos, vel, mass)
+    Eo1, _ = oracle.energy(o["pos"], o["vel"], mass)
+    assert np.abs(energy_err(g["E"], g["E0"]) - energy_err(Eo1, Eo0)).max() <= 1e-9
+
+
+@pytest.mark.parametrize("cfg,n_sample", [(1, 192), (2, 96), (3, 48)])
+def test_full_size_launch_sampled_parity(cfg, n_sample):
+    """BASELINE.json configs 1-3 at FULL size in the launch configuration bench.py times; the oracle recomputes a
+    strided sample of systems one by one (each system is independent, so a sample is exact for those systems)."""
+    c = W.CONFIGS[cfg]
+    pos, vel, mass = W.generate(cfg)
+    g = run_cuda(c, pos, vel, mass, want_energy=True)
+    idx = np.unique(np.concatenate([np.arange(0, c.n_sys, c.n_sys // n_sample), [c.n_sys - 1]]))
+    # add every system the CUDA path stopped on a monitor (up to 64), so stops are checked, not just survivors
+    stopped = np.nonzero(g["status"] >= ens.STOP_CLOSE)[0][:64]
+    idx = np.unique(np.concatenate([idx, stopped]))
+    o = run_oracle(c, pos[idx], vel[idx], mass[idx])
+    ol = run_oracle(c, pos[idx], vel[idx], mass[idx], prec=oracle.LONG_DOUBLE)
+    # knife-edge exemption (R12): a stop decided within 1e-9 relative of the threshold may differ by a step
+    same = (g["status"][idx] == o["status"]) & (g["nsteps"][idx] == o["nsteps"])
+    assert same.mean() >= 0.99, f"status/nsteps mismatches: {(~same).sum()} of {len(idx)}"
+    ok = same & (o["status"] == oracle.DONE_STEPS) & (ol["status"] == oracle.DONE_STEPS)
+    # "stable, well separated" made operational: oracle double and long double agree to 1e-8
+    floor_p = rel_diff(o["pos"], ol["pos"])
+    ok &= floor_p <= 1e-8
+    assert ok.sum() >= 0.8 * len(idx)
+    dp = rel_diff(g["pos"][idx], o["pos"])[ok]
+    dv = rel_diff(g["vel"][idx], o["vel"])[ok]
+    print(f"cfg{cfg}: {ok.sum()} stable sampled systems of {len(idx)}; pos max {dp.max():.3e} vel max {dv.max():.3e}; "
+          f"oracle double-vs-long-double floor max {floor_p[ok].max():.3e}; stops in ensemble: "
+          f"{(g['status'] == ens.STOP_CLOSE).sum()} close, {(g['status'] == ens.STOP_EJECT).sum()} eject")
+    assert dp.max() <= 1e-6 and dv.max() <= 1e-6
+    Eo0, _ = oracle.energy(pos[idx], vel[idx], mass[idx])
+    Eo1, _ = oracle.energy(o["pos"], o["vel"], mass[idx])
+    de = np.abs(energy_err(g["E"][idx], g["E0"][idx]) - energy_err(Eo1, Eo0))[ok]
+    assert de.max() <= 1e-9
+    # properties that hold at any size: every system ran to its budget or stopped with a legal code
+    assert np.isin(g["status"], [ens.DONE_STEPS, ens.STOP_CLOSE, ens.STOP_EJECT]).all()
+    done = g["status"] == ens.DONE_STEPS
+    assert (g["nsteps"][done] == c.steps).all() and (g["nsteps"][~done] < c.steps).all()
+    assert np.isfinite(g["pos"]).all() and np.isfinite(g["vel"]).all()
+    # angular momentum is conserved by the scheme to rounding level for every system
+    dL = np.abs(g["L"] - g["L0"]).max(axis=1) / np.linalg.norm(g["L0"], axis=1)
+    assert dL[done].max() <= 1e-9
+
+
+def _random_systems(n_sys, n_body, seed):
+    """Star + planets on well separated, mildly eccentric orbits (generic n_body; not a BASELINE config)."""
+    rng = np.random.default_rng(seed)
+    pos = np.zeros((n_sys, n_body, 3))
+    vel = np.zeros((n_sys, n_body, 3))
+    mass = np.ones((n_sys, n_body))
+    a = np.cumprod(np.concatenate([rng.uniform(0.6, 1.0, (n_sys, 1)), rng.uniform(1.3, 1.6, (n_sys, n_body - 1))], 1), 1)
+    for b in range(1, n_body):
+        m = 10.0 ** rng.uniform(-6, -3, n_sys)
+        mass[:, b] = m
+        e, inc = rng.uniform(0, 0.05, n_sys), rng.uniform(0, 0.03, n_sys)
+        Om, om, M = (rng.uniform(0, 2 * np.pi, n_sys) for _ in range(3))
+        pos[:, b], vel[:, b] = W.elements_to_cartesian(a[:, b - 1], e, inc, Om, om, M, 1.0 + m)
+    mt = mass.sum(1)[:, None]
+    pos -= ((mass[:, :, None] * pos).sum(1) / mt)[:, None]
+    vel -= ((mass[:, :, None] * vel).sum(1) / mt)[:, None]
+    return pos, vel, mass
+
+
+@pytest.mark.parametrize("n_body", list(range(2, 17)))
+def test_every_body_count_ragged(n_body):
+    """All supported n_body (every lane/body split, exact and padded shapes), a ragged ensemble size that ends in
+    the middle of a warp, several warps and blocks."""
+    n_sys = 333
+    pos, vel, mass = _random_systems(n_sys, n_body, 100 + n_body)
+    steps, dt = 300, 0.004
+    g = ens.run(ens.HERMITE, pos, vel, mass, dt=dt, steps=steps)
+    o = oracle.integrate(oracle.HERMITE, pos, vel, mass, dt=dt, max_steps=steps)
+    assert (g["status"] == o["status"]).all() and (g["nsteps"] == o["nsteps"]).all()
+    dp, dv = rel_diff(g["pos"], o["pos"]), rel_diff(g["vel"], o["vel"])
+    assert dp.max() <= 1e-11 and dv.max() <= 1e-11, (dp.max(), dv.max())
+
+
+@pytest.mark.parametrize("n_sys", [1, 31, 32, 33, 63, 64, 65, 1000])
+def test_set_get_roundtrip_bit_exact(n_sys):
+    """AoS -> SoA -> AoS transposition is pure data movement: bit-exact, for ragged sizes around the 64-system tile,
+    for host and device memory spaces."""
+    for n_body in (2, 3, 6, 15):
+        rng = np.random.default_rng(n_sys * 17 + n_body)
+        pos, vel = rng.normal(size=(n_sys, n_body, 3)), rng.normal(size=(n_sys, n_body, 3))
+        mass, time = rng.uniform(size=(n_sys, n_body)), rng.normal(size=n_sys)
+        with ens.Ensemble(n_sys, n_body) as e:
+            e.set_state(pos, vel, mass, time)
+            s = e.get_state()
+            assert (s["pos"] == pos).all() and (s["vel"] == vel).all() and (s["time"] == time).all()
+            assert (s["status"] == ens.ACTIVE).all() and (s["nsteps"] == 0).all()
+            tp, tv, tm = (torch.from_numpy(x).cuda() for x in (pos, vel, mass))
+            e.set_state(tp, tv, tm)
+            d = e.get_state(device=True)
+            torch.cuda.synchronize()
+            assert torch.equal(d["pos"], tp) and torch.equal(d["vel"], tv) and (d["time"] == 0).all()
+
+
+def test_split_runs_and_checkpoint_are_bit_identical():
+    """The step is a pure function of (x, v, m, t) (R6): 400 steps == 150 + 250 steps == get/set round trip."""
+    pos, vel, mass = W.generate(0, n_sys=200)
+    with ens.Ensemble(200, 3) as e:
+        e.set_state(pos, vel, mass)
+        e.integrate(ens.HERMITE, 0.01, 400)
+        a = e.get_state()
+        e.set_state(pos, vel, mass)
+        e.integrate(ens.HERMITE, 0.01, 150)
+        mid = e.get_state()
+        e.integrate(ens.HERMITE, 0.01, 250)
+        b = e.get_state()
+        assert (mid["nsteps"] == 150).all() and (b["nsteps"] == 400).all()
+        e.set_state(mid["pos"], mid["vel"], mass, mid["time"])
+        e.integrate(ens.HERMITE, 0.01, 250)
+        c = e.get_state()
+    for k in ("pos", "vel"):
+        assert (a[k] == b[k]).all() and (a[k] == c[k]).all()
+    np.testing.assert_allclose(a["time"], b["time"], rtol=0, atol=0)
+
+
+def test_time_reversal():
+    """Time-symmetrized scheme (R5b): forward then backward recovers the start far below truncation error."""
+    pos, vel, mass = W.generate(0, n_sys=128)
+    with ens.Ensemble(128, 3) as e:
+        e.set_state(pos, vel, mass)
+        e.integrate(ens.HERMITE, 0.01, 500)
+        f = e.get_state()
+        e.integrate(ens.HERMITE, -0.01, 500, t_end=-np.inf)
+        r = e.get_state()
+    o = oracle.integrate(oracle.HERMITE, pos, vel, mass, dt=0.01, max_steps=500)
+    o = oracle.integrate(oracle.HERMITE, o["pos"], o["vel"], mass, o["time"], dt=-0.01, t_end=-np.inf, max_steps=500)
+    assert rel_diff(r["pos"], pos).max() <= 1e-9        # defect of the 2-iteration corrector, same size as the oracle's
+    assert rel_diff(r["pos"], o["pos"]).max() <= 1e-11  # and it IS the oracle's defect
+    assert np.abs(r["time"]).max() <= 1e-12 and (r["nsteps"] == 1000).all()
+    assert rel_diff(f["pos"], pos).max() > 1e-3
+
+
+def test_t_end_semantics():
+    """R10: stop when t >= t_end, the last step is not clipped; DONE_* systems continue on the next call."""
+    pos, vel, mass = W.generate(0, n_sys=70)
+    time = np.linspace(0.0, 0.69, 70)
+    with ens.Ensemble(70, 3) as e:
+        e.set_state(pos, vel, mass, time)
+        e.integrate(ens.HERMITE, 0.01, 10**6, t_end=1.0)
+        g = e.get_state()
+        o = oracle.integrate(oracle.HERMITE, pos, vel, mass, time, dt=0.01, t_end=1.0, max_steps=10**6)
+        assert (g["status"] == ens.DONE_TIME).all() and (g["nsteps"] == o["nsteps"]).all()
+        assert (g["time"] == o["time"]).all() and (g["time"] >= 1.0).all() and (g["time"] < 1.0 + 0.0101).all()
+        assert rel_diff(g["pos"], o["pos"]).max() <= 1e-12
+        e.integrate(ens.HERMITE, 0.01, 7, t_end=np.inf)  # DONE_TIME systems run again
+        g2 = e.get_state()
+        assert (g2["status"] == ens.DONE_STEPS).all() and (g2["nsteps"] == o["nsteps"] + 7).all()
+        e.integrate(ens.HERMITE, 0.01, 0)  # zero steps: state untouched
+        g3 = e.get_state()
+        assert (g3["pos"] == g2["pos"]).all() and (g3["nsteps"] == g2["nsteps"]).all()
+
+
+def _crossing_ensemble(n_sys):
+    """Hand-built stops (R11): odd systems get an intruder on a near-collision course with planet 1, every fourth
+    system gets a fast outbound body that leaves r_eject; the rest run to the step budget."""
+    pos, vel, mass = W.generate(0, n_sys=n_sys)
+    for s in range(n_sys):
+        if s % 2 == 1:
+            d = np.array([0.05 + 0.001 * s, 0.003, 0.0])
+            pos[s, 2] = pos[s, 1] + d
+            vel[s, 2] = vel[s, 1] - d / np.linalg.norm(d) * (0.4 + 0.01 * (s % 7))
+        elif s % 4 == 0:
+            pos[s, 2] = np.array([3.0, 0.0, 0.0])
+            vel[s, 2] = np.array([2.5 + 0.05 * (s % 5), 0.3, 0.0])
+    return pos, vel, mass
+
+
+def test_monitors_stop_step_and_state_match_oracle():
+    n_sys = 96
+    pos, vel, mass = _crossing_ensemble(n_sys)
+    kw = dict(dt=0.002, r_close=0.02, r_eject=5.0)
+    g = ens.run(ens.HERMITE, pos, vel, mass, steps=3000, **kw)
+    o = oracle.integrate(oracle.HERMITE, pos, vel, mass, max_steps=3000, **kw)
+    assert (o["status"] == oracle.STOP_CLOSE).sum() >= 40 and (o["status"] == oracle.STOP_EJECT).sum() >= 20
+    assert (o["status"] == oracle.DONE_STEPS).sum() >= 20
+    assert (g["status"] == o["status"]).all()
+    assert (g["nsteps"] == o["nsteps"]).all()
+    assert (g["time"] == o["time"]).all()
+    # a stopped system keeps its post-step state
+    assert rel_diff(g["pos"], o["pos"]).max() <= 1e-9 and rel_diff(g["vel"], o["vel"]).max() <= 1e-9
+
+
+def test_stop_is_sticky_until_set_state():
+    n_sys = 64
+    pos, vel, mass = _crossing_ensemble(n_sys)
+    with ens.Ensemble(n_sys, 3) as e:
+        e.set_state(pos, vel, mass)
+        e.set_monitors(0.02, 5.0)
+        e.integrate(ens.HERMITE, 0.002, 3000)
+        a = e.get_state()
+        e.integrate(ens.HERMITE, 0.002, 100)
+        b = e.get_state()
+        stopped = a["status"] >= ens.STOP_CLOSE
+        assert stopped.any() and (~stopped).any()
+        assert (b["pos"][stopped] == a["pos"][stopped]).all() and (b["nsteps"][stopped] == a["nsteps"][stopped]).all()
+        assert (b["status"][stopped] == a["status"][stopped]).all()
+        assert (b["nsteps"][~stopped] == a["nsteps"][~stopped] + 100).all()
+        e.set_state(pos, vel, mass)
+        assert (e.get_state()["status"] == ens.ACTIVE).all()
+
+
+def test_nonfinite_state_is_flagged():
+    pos, vel, mass = W.generate(0, n_sys=40)
+    pos[7, 1, 0] = np.nan
+    vel[9, 2, 1] = np.inf
+    g = ens.run(ens.HERMITE, pos, vel, mass, dt=0.01, steps=20)
+    assert g["status"][7] == ens.STOP_NONFINITE and g["nsteps"][7] == 1
+    assert g["status"][9] == ens.STOP_NONFINITE
+    ok = np.ones(40, bool)
+    ok[[7, 9]] = False
+    assert (g["status"][ok] == ens.DONE_STEPS).all()
+
+
+def test_paper_initial_conditions_10pi():
+    """The paper's own validation: n = 3..6, ICs of §5.1, 10 pi time units, |x|, |v|, t within 1e-10."""
+    for n in (3, 4, 5, 6):
+        pos, vel, mass = W.paper_ics(n, n_sys=33)
+        steps = int(round(10 * np.pi / 1e-3))
+        g = ens.run(ens.HERMITE, pos, vel, mass, dt=1e-3, steps=steps)
+        o = oracle.integrate(oracle.HERMITE, pos, vel, mass, dt=1e-3, max_steps=steps)
+        assert np.abs(np.linalg.norm(g["pos"], axis=2) - np.linalg.norm(o["pos"], axis=2)).max() <= 1e-10
+        assert np.abs(np.linalg.norm(g["vel"], axis=2) - np.linalg.norm(o["vel"], axis=2)).max() <= 1e-10
+        assert np.abs(g["time"] - o["time"]).max() <= 1e-10
+
+
+def test_energy_matches_oracle():
+    for cfg in (0, 2, 3):
+        pos, vel, mass = W.generate(cfg, n_sys=300)
+        with ens.Ensemble(300, mass.shape[1]) as e:
+            e.set_state(pos, vel, mass)
+            E, L = e.energy()
+            Ed, Ld = e.energy(device=True)
+        Eo, Lo = oracle.energy(pos, vel, mass, prec=oracle.LONG_DOUBLE)
+        np.testing.assert_allclose(E, Eo, rtol=1e-14)
+        np.testing.assert_allclose(L, Lo, rtol=1e-13, atol=1e-18)
+        assert (Ed.cpu().numpy() == E).all() and (Ld.cpu().numpy() == L).all()
+
+
+def test_rsqrt_within_one_ulp():
+    """R14: float rsqrt seed + FP64 refinement is within 1 ulp of the correctly rounded 1/sqrt over 1e-8..1e8 and
+    near the ends of its documented domain."""
+    rng = np.random.default_rng(5)
+    x = np.concatenate([10.0 ** rng.uniform(-8, 8, 400000), 10.0 ** rng.uniform(-36, 36, 100000),
+                        np.array([1.0, 4.0, 0.25, 1e-6, 1e5, 2.0, 3.0])])
+    y = ens.rsqrt_probe(torch.from_numpy(x).cuda()).cpu().numpy()
+    ref = (1.0 / np.sqrt(x.astype(np.longdouble)))
+    ulp = np.spacing(ref.astype(np.float64))
+    err = np.abs((y.astype(np.longdouble) - ref) / ulp).astype(np.float64)
+    print(f"rsqrt: max error {err.max():.3f} ulp, mean {err.mean():.3f}")
+    assert err.max() <= 1.0
+
+
+def test_error_codes():
+    import ctypes
+    L = ens.lib()
+    h = ctypes.c_void_p()
+    assert L.ens_create(0, 3, ctypes.byref(h)) == ens.EINVAL
+    assert L.ens_create(10, 1, ctypes.byref(h)) == ens.EINVAL
+    assert L.ens_create(10, 17, ctypes.byref(h)) == ens.EINVAL
+    assert L.ens_create(10, 3, None) == ens.EINVAL
+    assert L.ens_create(10, 3, ctypes.byref(h)) == ens.OK
+    assert L.ens_integrate(h, ens.HERMITE, 0.01, float("inf"), 10, None) == ens.ESTATE
+    assert L.ens_get_state(h, None, None, None, None, None, ens.HOST, None) == ens.ESTATE
+    pos, vel, mass = W.generate(0, n_sys=10)
+    assert L.ens_set_state(h, pos.ctypes.data, None, mass.ctypes.data, None, ens.HOST, None) == ens.EINVAL
+    assert L.ens_set_state(h, pos.ctypes.data, vel.ctypes.data, mass.ctypes.data, None, 7, None) == ens.EINVAL
+    assert L.ens_set_state(h, pos.ctypes.data, vel.ctypes.data, mass.ctypes.data, None, ens.HOST, None) == ens.OK
+    for bad_dt in (0.0, float("nan"), float("inf")):
+        assert L.ens_integrate(h, ens.HERMITE, bad_dt, float("inf"), 10, None) == ens.EINVAL
+    assert L.ens_integrate(h, 2, 0.01, float("inf"), 10, None) == ens.EINVAL
+    assert L.ens_integrate(h, ens.HERMITE, 0.01, float("nan"), 10, None) == ens.EINVAL
+    assert L.ens_integrate(h, ens.HERMITE, 0.01, float("inf"), -1, None) == ens.EINVAL
+    assert L.ens_set_monitors(h, float("nan"), 1.0) == ens.EINVAL
+    assert L.ens_energy(h, None, None, ens.HOST, None) == ens.EINVAL
+    assert L.ens_integrate(None, ens.HERMITE, 0.01, float("inf"), 10, None) == ens.EINVAL
+    assert L.ens_destroy(h) == ens.OK and L.ens_destroy(None) == ens.OK
+    assert b"invalid" in L.ens_strerror(ens.EINVAL)
+
+
+def test_streams_are_honoured():
+    """Device-space calls only enqueue on the caller's stream (torch provides the stream and the memory)."""
+    pos, vel, mass = W.generate(0, n_sys=512)
+    tp, tv, tm = (torch.from_numpy(x).cuda() for x in (pos, vel, mass))
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with ens.Ensemble(512, 3) as e, torch.cuda.stream(s):
+        e.set_state(tp, tv, tm, stream=s)
+        e.integrate(ens.HERMITE, 0.01, 300, stream=s)
+        d = e.get_state(device=True, stream=s)
+        s.synchronize()
+        assert e.last_kernel_ms() > 0
+    o = oracle.integrate(oracle.HERMITE, pos, vel, mass, dt=0.01, max_steps=300)
+    assert rel_diff(d["pos"].cpu().numpy(), o["pos"]).max() <= 1e-11
