@@ -38,10 +38,10 @@ def test_full_size_launch_sampled_parity(cfg, n_sample):
     c = W.CONFIGS[cfg]
     pos, vel, mass = W.generate(cfg)
     g = run_cuda(c, pos, vel, mass, want_energy=True)
-    idx = np.unique(np.concatenate([np.arange(0, c.n_sys, c.n_sys // n_sample), [c.n_sys - 1]]))
+    strided = np.unique(np.concatenate([np.arange(0, c.n_sys, c.n_sys // n_sample), [c.n_sys - 1]]))
     # add every system the CUDA path stopped on a monitor (up to 64), so stops are checked, not just survivors
     stopped = np.nonzero(g["status"] >= ens.STOP_CLOSE)[0][:64]
-    idx = np.unique(np.concatenate([idx, stopped]))
+    idx = np.unique(np.concatenate([strided, stopped]))
     o = run_oracle(c, pos[idx], vel[idx], mass[idx])
     ol = run_oracle(c, pos[idx], vel[idx], mass[idx], prec=oracle.LONG_DOUBLE)
     # knife-edge exemption (R12): a stop decided within 1e-9 relative of the threshold may differ by a step
@@ -51,7 +51,7 @@ def test_full_size_launch_sampled_parity(cfg, n_sample):
     # "stable, well separated" made operational: oracle double and long double agree to 1e-8
     floor_p = rel_diff(o["pos"], ol["pos"])
     ok &= floor_p <= 1e-8
-    assert ok.sum() >= 0.8 * len(idx)
+    assert ok[np.isin(idx, strided)].sum() >= 0.8 * len(strided)  # most of the unbiased sample is stable
     dp = rel_diff(g["pos"][idx], o["pos"])[ok]
     dv = rel_diff(g["vel"][idx], o["vel"])[ok]
     print(f"cfg{cfg}: {ok.sum()} stable sampled systems of {len(idx)}; pos max {dp.max():.3e} vel max {dv.max():.3e}; "
