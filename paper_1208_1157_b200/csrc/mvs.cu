@@ -1,6 +1,90 @@
-// mvs.cu — placeholder until the MVS kernel lands (next commit): ens_integrate(ENS_MVS) returns ENS_EUNSUPPORTED.
-#include "ens_internal.cuh"
+// mvs.cu — instantiations of the fused MVS step-loop kernel and the n_body -> (L, B) dispatch.
+#include "mvs_kernel.cuh"
+
 namespace ensd {
-KernelInfo mvs_kernel_for(int) { KernelInfo k; k.fn = nullptr; k.shape.L = k.shape.B = 0; k.threads = 0; return k; }
-cudaError_t launch_mvs(const View&, const StepArgs&, int, cudaStream_t, int64_t*) { return cudaErrorNotSupported; }
+
+namespace {
+
+// n_body -> lanes per system L (odd), planets per lane B, L * B >= n_body - 1 (the star is held by every lane).
+template <int N> struct MvsShape;
+#define ENS_MVS_SHAPE(N_, L_, B_, THREADS_, MINB_)                             \
+    template <> struct MvsShape<N_> {                                          \
+        static constexpr int L = L_, B = B_, THREADS = THREADS_, MINB = MINB_; \
+    };
+//            N   L  B  threads minBlocks
+ENS_MVS_SHAPE(2, 1, 1, 128, 1)
+ENS_MVS_SHAPE(3, 1, 2, 128, 1)
+ENS_MVS_SHAPE(4, 1, 3, 128, 1)
+ENS_MVS_SHAPE(5, 1, 4, 128, 1)
+ENS_MVS_SHAPE(6, 1, 5, 128, 1)
+ENS_MVS_SHAPE(7, 3, 2, 128, 1)
+ENS_MVS_SHAPE(8, 3, 3, 128, 1)
+ENS_MVS_SHAPE(9, 3, 3, 128, 1)
+ENS_MVS_SHAPE(10, 3, 3, 128, 1)
+ENS_MVS_SHAPE(11, 5, 2, 128, 1)
+ENS_MVS_SHAPE(12, 3, 4, 128, 1)
+ENS_MVS_SHAPE(13, 3, 4, 128, 1)
+ENS_MVS_SHAPE(14, 5, 3, 128, 1)
+ENS_MVS_SHAPE(15, 5, 3, 128, 1)
+ENS_MVS_SHAPE(16, 5, 3, 128, 1)
+#undef ENS_MVS_SHAPE
+
+template <int N>
+constexpr auto kernel_ptr() {
+    using S = MvsShape<N>;
+    return &mvs_kernel<N, S::L, S::B, 128, S::MINB>;
 }
+
+template <int N>
+KernelInfo info_of() {
+    using S = MvsShape<N>;
+    KernelInfo k;
+    k.fn = (const void*)kernel_ptr<N>();
+    k.shape.L = S::L;
+    k.shape.B = S::B;
+    k.threads = S::THREADS;
+    return k;
+}
+
+template <int N>
+cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
+    using S = MvsShape<N>;
+    if (threads > 128) threads = 128;  // __launch_bounds__ of the kernel
+    const int64_t sys_per_warp = 32 / S::L;
+    const int64_t warps = (v.n_sys + sys_per_warp - 1) / sys_per_warp;
+    const int wpb = threads / 32;
+    const int64_t blocks = (warps + wpb - 1) / wpb;
+    if (blocks_out) *blocks_out = blocks;
+    kernel_ptr<N>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+#define ENS_FOR_EACH_N(X) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
+
+KernelInfo mvs_kernel_for(int n_body) {
+    switch (n_body) {
+#define X(N_) \
+    case N_: return info_of<N_>();
+        ENS_FOR_EACH_N(X)
+#undef X
+    }
+    KernelInfo none;
+    none.fn = nullptr;
+    none.shape.L = none.shape.B = 0;
+    none.threads = 0;
+    return none;
+}
+
+cudaError_t launch_mvs(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
+    switch (v.n_body) {
+#define X(N_) \
+    case N_: return launch_n<N_>(v, a, threads, s, blocks_out);
+        ENS_FOR_EACH_N(X)
+#undef X
+    }
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace ensd

@@ -1,0 +1,440 @@
+// mvs_kernel.cuh — the fused mixed-variable-symplectic step loop for sm_100a (FP64 CUDA cores).
+//
+// One launch = Alg. 1 for every system with the MVS propagator of P:L99-125 / P:L254-256 in
+// democratic-heliocentric variables (reading R-M1: heliocentric positions Q_i = x_i - x_0, barycentric velocities
+// V_i = v_i - V_cm, centre of mass X_cm, V_cm).  The state is converted once at load, lives in registers for all
+// steps, and is converted back once at store.  One step (five sub-steps, kept unmerged, R-M7):
+//   1  Q_i += h/2 s,  s = sum_k m_k V_k / m_0;  X_cm += h/2 V_cm          Cartesian drift
+//   2  V_i += h/2 A_i                                                     kick, planets only
+//   3  (Q_i, V_i) <- Kepler flow about mu = G m_0 for h                   Kepler drift             (R-M2)
+//   4  A = planet-planet accelerations at the new Q, each pair once       (reused by step k+1's sub-step 2,
+//      V_i += h/2 A_i                                                      P:L256)
+//   5  Q_i += h/2 s (s from the new V; the SAME s opens the next step), X_cm += h/2 V_cm
+// The Kepler drift uses universal variables (BASELINE.json config 4; R-M3, R-M4): solve
+//   r0 G1 + eta G2 + mu G3 = tau,  G_n = X^n c_n(beta X^2),  by Newton from X = tau / r0, then the f and g functions.
+//
+// Work split: L lanes per system (L odd), B planets per lane; the Kepler drift is per planet and needs no
+// communication; planet-planet pairs use the same in-lane + ring-of-shuffles schedule as the Hermite kernel; the
+// momentum sum of the Cartesian drift is an L-lane all-gather of per-lane partial sums.  L = 1 (n_body <= 6) is
+// one system per thread with the oracle's summation order and no shuffle.
+#pragma once
+#include <cfloat>
+
+#include "ens_device.cuh"
+
+namespace ensd {
+
+// Stumpff functions c_n(z) = sum_k (-z)^k / (2k+n)!  (R-M3).  |z| is quartered until <= 0.1, the series is summed
+// there (8 terms: truncation < 1e-21 relative), and c_n(4z) is rebuilt from c_n(z) by the duplication formulas.
+// For the step sizes of the workloads (h << orbital period) z = beta X^2 is small and both loops run zero times.
+__device__ __forceinline__ void stumpff(double z, double& c0, double& c1, double& c2, double& c3) {
+    int nq = 0;
+    while (fabs(z) > 0.1) {
+        z *= 0.25;
+        ++nq;
+    }
+    double s2 = -1.0 / 20922789888000.0;    // -1/16!
+    double s3 = -1.0 / 355687428096000.0;   // -1/17!
+    s2 = fma(s2, z, 1.0 / 87178291200.0);   //  1/14!
+    s3 = fma(s3, z, 1.0 / 1307674368000.0); //  1/15!
+    s2 = fma(s2, z, -1.0 / 479001600.0);    // -1/12!
+    s3 = fma(s3, z, -1.0 / 6227020800.0);   // -1/13!
+    s2 = fma(s2, z, 1.0 / 3628800.0);       //  1/10!
+    s3 = fma(s3, z, 1.0 / 39916800.0);      //  1/11!
+    s2 = fma(s2, z, -1.0 / 40320.0);        // -1/8!
+    s3 = fma(s3, z, -1.0 / 362880.0);       // -1/9!
+    s2 = fma(s2, z, 1.0 / 720.0);           //  1/6!
+    s3 = fma(s3, z, 1.0 / 5040.0);          //  1/7!
+    s2 = fma(s2, z, -1.0 / 24.0);           // -1/4!
+    s3 = fma(s3, z, -1.0 / 120.0);          // -1/5!
+    c2 = fma(s2, z, 0.5);                   //  1/2!
+    c3 = fma(s3, z, 1.0 / 6.0);             //  1/3!
+    c1 = fma(-z, c3, 1.0);
+    c0 = fma(-z, c2, 1.0);
+    for (; nq > 0; --nq) {
+        const double n3 = 0.25 * fma(c0, c3, c2);
+        const double n2 = 0.5 * c1 * c1;
+        const double n1 = c0 * c1;
+        const double n0 = fma(2.0 * c0, c0, -1.0);
+        c3 = n3;
+        c2 = n2;
+        c1 = n1;
+        c0 = n0;
+    }
+}
+
+struct KeplerG {
+    double G0, G1, G2, G3;
+};
+
+__device__ __forceinline__ KeplerG kepler_G(double beta, double X) {
+    const double X2 = X * X;
+    double c0, c1, c2, c3;
+    stumpff(beta * X2, c0, c1, c2, c3);
+    KeplerG g;
+    g.G0 = c0;
+    g.G1 = X * c1;
+    g.G2 = X2 * c2;
+    g.G3 = (X2 * X) * c3;
+    return g;
+}
+
+// Residual of the universal Kepler equation; monotone in X (its derivative is the radius r > 0).
+__device__ __forceinline__ double kepler_resid(double r0, double eta, double mu, double beta, double tau, double X) {
+    const KeplerG g = kepler_G(beta, X);
+    return fma(r0, g.G1, fma(eta, g.G2, fma(mu, g.G3, -tau)));
+}
+
+// Guaranteed-convergent fallback (R-M4): bracket the root and bisect.  Out of line: essentially never taken.
+__device__ __noinline__ double kepler_bisect(double r0, double eta, double mu, double beta, double tau) {
+    double lo = 0.0, hi = tau / r0;
+    const double sgn = tau >= 0.0 ? 1.0 : -1.0;
+    if (hi == 0.0) hi = sgn;
+    for (int k = 0; k < 200 && sgn * kepler_resid(r0, eta, mu, beta, tau, hi) < 0.0; ++k) hi *= 2.0;
+    for (int k = 0; k < 200; ++k) {
+        const double mid = 0.5 * (lo + hi);
+        if (sgn * kepler_resid(r0, eta, mu, beta, tau, mid) < 0.0)
+            lo = mid;
+        else
+            hi = mid;
+    }
+    return 0.5 * (lo + hi);
+}
+
+// Advance (q, p) along the Kepler orbit about a fixed centre of gravitational parameter mu for time tau.
+__device__ __forceinline__ void kepler_drift(double (&q)[3], double (&p)[3], double mu, double tau) {
+    const double r0 = sqrt(fma(q[2], q[2], fma(q[1], q[1], q[0] * q[0])));
+    const double eta = fma(q[2], p[2], fma(q[1], p[1], q[0] * p[0]));
+    const double v2 = fma(p[2], p[2], fma(p[1], p[1], p[0] * p[0]));
+    const double beta = 2.0 * mu / r0 - v2;
+    double X = tau / r0;
+    bool ok = false;
+    for (int it = 0; it < 50; ++it) {
+        const KeplerG g = kepler_G(beta, X);
+        const double F = fma(r0, g.G1, fma(eta, g.G2, fma(mu, g.G3, -tau)));
+        const double dF = fma(r0, g.G0, fma(eta, g.G1, mu * g.G2));
+        const double dX = F / dF;
+        X -= dX;
+        if (!(fabs(dX) > 1e-15 * fabs(X))) {
+            ok = true;
+            break;
+        }
+    }
+    if (!ok || !(fabs(X) <= DBL_MAX)) X = kepler_bisect(r0, eta, mu, beta, tau);
+    const KeplerG g = kepler_G(beta, X);
+    const double r = fma(r0, g.G0, fma(eta, g.G1, mu * g.G2));
+    const double f = 1.0 - mu * g.G2 / r0;
+    const double gg = fma(-mu, g.G3, tau);
+    const double fd = -mu * g.G1 / (r0 * r);
+    const double gd = 1.0 - mu * g.G2 / r;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double qn = fma(f, q[c], gg * p[c]);
+        const double pn = fma(fd, q[c], gd * p[c]);
+        q[c] = qn;
+        p[c] = pn;
+    }
+}
+
+// One unordered planet pair (i, k), acceleration only: a_i += m_k dx / r^3, a_k -= m_i dx / r^3  (Eq. 1, R1).
+__device__ __forceinline__ double pair_acc(const double (&xi)[3], double mi, double (&ai)[3], const double (&xk)[3],
+                                           double mk, double (&ak)[3]) {
+    double dx[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dx[c] = xk[c] - xi[c];
+    const double r2 = fma(dx[2], dx[2], fma(dx[1], dx[1], dx[0] * dx[0]));
+    const double y = rsqrt_f64(r2);
+    const double y3 = y * y * y;
+    const double wi = mk * y3;
+    const double wk = -mi * y3;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        ai[c] = fma(wi, dx[c], ai[c]);
+        ak[c] = fma(wk, dx[c], ak[c]);
+    }
+    return r2;
+}
+
+// Planet-planet accelerations of the B planets this lane owns (the star's pull is in the Kepler drift).
+// In-lane pairs in (b ascending, c ascending) order give every planet its contributions in ascending k, the
+// oracle's order, when L = 1.
+template <int P, int L, int B>
+__device__ __forceinline__ void eval_acc_planets(const double (&Q)[B][3], const double (&m)[B], double (&A)[B][3],
+                                                 u64& r2min, int l, int base, unsigned amask) {
+    constexpr bool PADDED = (L * B != P);
+#pragma unroll
+    for (int b = 0; b < B; ++b) A[b][0] = A[b][1] = A[b][2] = 0.0;
+    r2min = ~0ull;
+#pragma unroll
+    for (int b = 0; b < B; ++b)
+#pragma unroll
+        for (int c = b + 1; c < B; ++c) {
+            const double r2 = pair_acc(Q[b], m[b], A[b], Q[c], m[c], A[c]);
+            min_bits(r2min, r2, !PADDED || (l * B + c < P));
+        }
+    if constexpr (L > 1) {
+#pragma unroll
+        for (int s = 1; s <= (L - 1) / 2; ++s) {
+            int ls = l + s;
+            if (ls >= L) ls -= L;
+            int lr = l - s;
+            if (lr < 0) lr += L;
+            const int src = base + ls, ret = base + lr;
+#pragma unroll
+            for (int c = 0; c < B; ++c) {
+                double xv[3], av[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+                for (int q = 0; q < 3; ++q) xv[q] = __shfl_sync(amask, Q[c][q], src);
+                const double mv = __shfl_sync(amask, m[c], src);
+                const bool vvalid = !PADDED || (ls * B + c < P);
+#pragma unroll
+                for (int b = 0; b < B; ++b) {
+                    const double r2 = pair_acc(Q[b], m[b], A[b], xv, mv, av);
+                    min_bits(r2min, r2, vvalid && (!PADDED || (l * B + b < P)));
+                }
+#pragma unroll
+                for (int q = 0; q < 3; ++q) A[c][q] += __shfl_sync(amask, av[q], ret);
+            }
+        }
+    }
+}
+
+// sum over the planets of the system of m_k W_k (W = V or Q).  L = 1: ascending k, the oracle's order.
+// L > 1: per-lane partial sums, gathered from the lanes of the system in lane order.
+template <int L, int B>
+__device__ __forceinline__ void mass_weighted_sum(const double (&W)[B][3], const double (&m)[B], double (&out)[3], int l,
+                                                  int base, unsigned amask) {
+    double part[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+    for (int b = 0; b < B; ++b)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) part[c] = fma(m[b], W[b][c], part[c]);  // dummy slots have m = 0
+    if constexpr (L == 1) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) out[c] = part[c];
+    } else {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double acc = __shfl_sync(amask, part[c], base);
+#pragma unroll
+            for (int i = 1; i < L; ++i) acc += __shfl_sync(amask, part[c], base + i);
+            out[c] = acc;
+        }
+    }
+}
+
+template <int N, int L, int B, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) mvs_kernel(View e, StepArgs p) {
+    constexpr int P = N - 1;   // planets; body 0 is the star
+    constexpr int S = 32 / L;  // systems per warp
+    constexpr bool PADDED = (L * B != P);
+    const int lane = threadIdx.x & 31;
+    const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int sl = lane / L;
+    const int l = lane - sl * L;
+    const int base = sl * L;
+    const int64_t sys = warp * S + sl;
+    const bool live = (sl < S) && (sys < e.n_sys);
+
+    double Q[B][3], V[B][3], A[B][3], m[B];
+    double Xcm[3] = {0.0, 0.0, 0.0}, Vcm[3] = {0.0, 0.0, 0.0};
+    double m0 = 1.0, Mtot = 1.0, t = 0.0;
+    int st = ENS_STOP_NONFINITE;
+    bool active = false;
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+        // dummy slot (padded shapes only): massless, far from everything and from each other; never drifted
+        Q[b][0] = 1.0e8 * (double)(l * B + b + 2);
+        Q[b][1] = Q[b][2] = 0.0;
+        V[b][0] = V[b][1] = V[b][2] = 0.0;
+        m[b] = 0.0;
+    }
+    if (live) {
+        st = e.status[sys];
+        active = st < ENS_STOP_CLOSE;  // STOP_* are sticky; DONE_* run again
+        t = e.time[sys];
+        // to_dh: total mass and centre of mass over all bodies in index order; every lane of the system reads all
+        // bodies (L1-resident, once per launch) so that the sums need no communication
+        double x0[3], sx[3] = {0.0, 0.0, 0.0}, sv[3] = {0.0, 0.0, 0.0};
+        Mtot = 0.0;
+#pragma unroll
+        for (int i = 0; i < N; ++i) {
+            const double mi = e.mass[(int64_t)i * e.n_pad + sys];
+            Mtot += mi;
+            if (i == 0) m0 = mi;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double xi = e.pos[(int64_t)(i * 3 + c) * e.n_pad + sys];
+                const double vi = e.vel[(int64_t)(i * 3 + c) * e.n_pad + sys];
+                if (i == 0) x0[c] = xi;
+                sx[c] = fma(mi, xi, sx[c]);
+                sv[c] = fma(mi, vi, sv[c]);
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            Xcm[c] = sx[c] / Mtot;
+            Vcm[c] = sv[c] / Mtot;
+        }
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const int body = l * B + b + 1;
+            if (!PADDED || body < N) {
+                m[b] = e.mass[(int64_t)body * e.n_pad + sys];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    Q[b][c] = e.pos[(int64_t)(body * 3 + c) * e.n_pad + sys] - x0[c];
+                    V[b][c] = e.vel[(int64_t)(body * 3 + c) * e.n_pad + sys] - Vcm[c];
+                }
+            }
+        }
+    }
+    const bool writeback = active;
+
+    const double h = p.dt, hh = 0.5 * p.dt;
+    const bool fwd = h > 0.0;
+    const bool mon_close = p.rc2_bits != 0ull;
+    const bool mon_eject = p.re2_bits < 0x7FEFFFFFFFFFFFFFull;
+    int64_t k = 0;
+    u64 r2min = ~0ull;
+    double s[3] = {0.0, 0.0, 0.0};
+
+    // Alg. 1 loop test before the first step (R10): time first, then the step budget
+    if (active) {
+        if (!(fwd ? (t < p.t_end) : (t > p.t_end))) {
+            st = ENS_DONE_TIME;
+            active = false;
+        } else if (k >= p.max_steps) {
+            st = ENS_DONE_STEPS;
+            active = false;
+        }
+    }
+    {  // prepare(P) (Alg. 1): accelerations and drift velocity of the initial state
+        const unsigned amask = __ballot_sync(0xffffffffu, active);
+        if (active) {
+            eval_acc_planets<P, L, B>(Q, m, A, r2min, l, base, amask);
+            mass_weighted_sum<L, B>(V, m, s, l, base, amask);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) s[c] = s[c] / m0;
+        }
+    }
+
+    while (true) {
+        const unsigned amask = __ballot_sync(0xffffffffu, active);
+        if (amask == 0) break;
+        if (active) {
+            // 1 + 2: Cartesian half drift, half kick
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double sh = hh * s[c];
+#pragma unroll
+                for (int b = 0; b < B; ++b) {
+                    Q[b][c] += sh;
+                    V[b][c] = fma(hh, A[b][c], V[b][c]);
+                }
+                Xcm[c] = fma(hh, Vcm[c], Xcm[c]);
+            }
+            // 3: Kepler drift of every planet about mu = G m_0 (G = 1)
+#pragma unroll
+            for (int b = 0; b < B; ++b)
+                if (!PADDED || (l * B + b < P)) kepler_drift(Q[b], V[b], m0, h);
+            // 4: planet-planet accelerations at the new positions, half kick
+            eval_acc_planets<P, L, B>(Q, m, A, r2min, l, base, amask);
+#pragma unroll
+            for (int b = 0; b < B; ++b)
+#pragma unroll
+                for (int c = 0; c < 3; ++c) V[b][c] = fma(hh, A[b][c], V[b][c]);
+            // 5: Cartesian half drift with the new momenta
+            mass_weighted_sum<L, B>(V, m, s, l, base, amask);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                s[c] = s[c] / m0;
+                const double sh = hh * s[c];
+#pragma unroll
+                for (int b = 0; b < B; ++b) Q[b][c] += sh;
+                Xcm[c] = fma(hh, Vcm[c], Xcm[c]);
+            }
+            t += h;
+            ++k;
+
+            // monitors on the post-step state (Alg. 1 execute(M); R11).  Planet-planet separations are
+            // those of the acceleration evaluation: the drift shifts every planet alike.
+            int f = 0;
+            double sq[3] = {0.0, 0.0, 0.0};
+            if (mon_eject) mass_weighted_sum<L, B>(Q, m, sq, l, base, amask);
+            double x0[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) x0[c] = Xcm[c] - sq[c] / Mtot;
+            if (mon_close && r2min < p.rc2_bits) f |= 1;
+            if (mon_eject && dbits(fma(x0[2], x0[2], fma(x0[1], x0[1], x0[0] * x0[0]))) > p.re2_bits) f |= 2;
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                if (!PADDED || (l * B + b < P)) {
+                    const u64 q2 = dbits(fma(Q[b][2], Q[b][2], fma(Q[b][1], Q[b][1], Q[b][0] * Q[b][0])));
+                    if (q2 > 0x7FEFFFFFFFFFFFFFull) f |= 4;  // +inf or NaN
+                    if (q2 < p.rc2_bits) f |= 1;             // star-planet separation is |Q_i|
+                    if (mon_eject) {
+                        const double xx = x0[0] + Q[b][0], yy = x0[1] + Q[b][1], zz = x0[2] + Q[b][2];
+                        if (dbits(fma(zz, zz, fma(yy, yy, xx * xx))) > p.re2_bits) f |= 2;
+                    }
+                }
+            }
+            if constexpr (L > 1) {
+                int g = f;
+#pragma unroll
+                for (int i = 1; i < L; ++i) {
+                    int li = l + i;
+                    if (li >= L) li -= L;
+                    g |= __shfl_sync(amask, f, base + li);
+                }
+                f = g;
+            }
+            if (f) {
+                st = (f & 4) ? ENS_STOP_NONFINITE : (f & 1) ? ENS_STOP_CLOSE : ENS_STOP_EJECT;
+                active = false;
+            } else if (!(fwd ? (t < p.t_end) : (t > p.t_end))) {
+                st = ENS_DONE_TIME;
+                active = false;
+            } else if (k >= p.max_steps) {
+                st = ENS_DONE_STEPS;
+                active = false;
+            }
+        }
+    }
+
+    // from_dh and store.  All lanes of a system left the loop together (t, k and the monitor flags are replicated).
+    const unsigned wmask = __ballot_sync(0xffffffffu, writeback);
+    if (writeback) {
+        double sq[3], sp[3], x0[3], v0[3];
+        mass_weighted_sum<L, B>(Q, m, sq, l, base, wmask);
+        mass_weighted_sum<L, B>(V, m, sp, l, base, wmask);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            x0[c] = Xcm[c] - sq[c] / Mtot;
+            v0[c] = Vcm[c] - sp[c] / m0;
+        }
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const int body = l * B + b + 1;
+            if (!PADDED || body < N) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    e.pos[(int64_t)(body * 3 + c) * e.n_pad + sys] = x0[c] + Q[b][c];
+                    e.vel[(int64_t)(body * 3 + c) * e.n_pad + sys] = V[b][c] + Vcm[c];
+                }
+            }
+        }
+        if (l == 0) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                e.pos[(int64_t)c * e.n_pad + sys] = x0[c];
+                e.vel[(int64_t)c * e.n_pad + sys] = v0[c];
+            }
+            e.time[sys] = t;
+            e.status[sys] = st;
+            e.nsteps[sys] += k;
+        }
+    }
+}
+
+}  // namespace ensd
