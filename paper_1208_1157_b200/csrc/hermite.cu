@@ -8,14 +8,28 @@ namespace {
 // n_body -> lanes per system L (odd), bodies per lane B, L * B >= n_body.  Exact fits for 2-6, 9, 10, 12, 15;
 // the others run in the next larger shape with massless dummy slots.
 template <int N> struct ShapeOf;
-#define ENS_SHAPE(N_, L_, B_, UNROLL_, THREADS_, MINB_)                 \
-    template <> struct ShapeOf<N_> {                                    \
-        static constexpr int L = L_, B = B_, THREADS = THREADS_, MINB = MINB_; \
-        static constexpr bool UNROLL = UNROLL_;                         \
+#define ENS_SHAPE(N_, L_, B_, UNROLL_, THREADS_, MINB_) ENS_SHAPE_T(N_, L_, B_, UNROLL_, THREADS_, MINB_, 128)
+#define ENS_SHAPE_T(N_, L_, B_, UNROLL_, THREADS_, MINB_, MAXT_)                        \
+    template <> struct ShapeOf<N_> {                                                    \
+        static constexpr int L = L_, B = B_, THREADS = THREADS_, MINB = MINB_, MAXT = MAXT_; \
+        static constexpr bool UNROLL = UNROLL_;                                         \
     };
+// Tuning knobs of the headline shape (n_body = 3), overridable at compile time for the sweeps recorded in DESIGN.md §8.
+#ifndef ENS_H3_UNROLL
+#define ENS_H3_UNROLL true
+#endif
+#ifndef ENS_H3_THREADS
+#define ENS_H3_THREADS 64
+#endif
+#ifndef ENS_H3_MAXT
+#define ENS_H3_MAXT 64  // __launch_bounds__ threads: with MINB it sets the register cap 65536 / (MAXT * MINB)
+#endif
+#ifndef ENS_H3_MINB
+#define ENS_H3_MINB 7  // 128 registers, no spills, 8 blocks of 2 warps per SM: 43.9 ms vs 48.1 ms at 188 registers
+#endif
 //        N  L  B  unroll threads minBlocks
 ENS_SHAPE(2, 1, 2, true, 64, 1)
-ENS_SHAPE(3, 1, 3, true, 64, 1)
+ENS_SHAPE_T(3, 1, 3, ENS_H3_UNROLL, ENS_H3_THREADS, ENS_H3_MINB, ENS_H3_MAXT)
 ENS_SHAPE(4, 1, 4, false, 64, 1)
 ENS_SHAPE(5, 1, 5, false, 64, 1)
 ENS_SHAPE(6, 3, 2, false, 64, 1)
@@ -30,11 +44,12 @@ ENS_SHAPE(14, 5, 3, false, 64, 1)
 ENS_SHAPE(15, 5, 3, false, 64, 1)
 ENS_SHAPE(16, 5, 4, false, 64, 1)
 #undef ENS_SHAPE
+#undef ENS_SHAPE_T
 
 template <int N>
 constexpr auto kernel_ptr() {
     using S = ShapeOf<N>;
-    return &hermite_kernel<N, S::L, S::B, S::UNROLL, 128, S::MINB>;
+    return &hermite_kernel<N, S::L, S::B, S::UNROLL, S::MAXT, S::MINB>;
 }
 
 template <int N>
@@ -51,7 +66,7 @@ KernelInfo info_of() {
 template <int N>
 cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
     using S = ShapeOf<N>;
-    if (threads > 128) threads = 128;  // __launch_bounds__ of the kernel
+    if (threads > S::MAXT) threads = S::MAXT;  // __launch_bounds__ of the kernel
     const int64_t sys_per_warp = 32 / S::L;
     const int64_t warps = (v.n_sys + sys_per_warp - 1) / sys_per_warp;
     const int wpb = threads / 32;
