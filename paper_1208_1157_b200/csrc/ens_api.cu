@@ -319,6 +319,7 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
     if (!(re2 < DBL_MAX)) re2 = DBL_MAX;
     memcpy(&a.rc2_bits, &rc2, 8);
     memcpy(&a.re2_bits, &re2, 8);
+    ensd::fill_step_constants(a);
     const ensd::KernelInfo& ki = integrator == ENS_HERMITE ? e->hermite : e->mvs;
     if (!ki.fn) return ENS_EUNSUPPORTED;
     const int threads = e->threads_override ? e->threads_override : ki.threads;

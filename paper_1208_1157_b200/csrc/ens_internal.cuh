@@ -30,7 +30,27 @@ struct StepArgs {
     int64_t max_steps;
     unsigned long long rc2_bits;  // bit pattern of r_close^2 (0 when the monitor is off)
     unsigned long long re2_bits;  // bit pattern of min(r_eject^2, DBL_MAX): also catches inf / NaN positions
+    // Step-size powers of Eq. 3 / Eq. 4 folded into per-launch constants (hermite_kernel.cuh), computed once on the
+    // host in IEEE double and read by the kernels straight from the constant bank (no registers held across the loop):
+    //   x_p = x + h v + p_a a0 + p_j j0              v_p = v + h a0 + p_a j0
+    //   C_x = x + h v + cx_a a0 + cx_j j0            C_v = v + cv_a a0 + cv_j j0
+    //   x_c = C_x + kx_a a1 + kx_j j1                v_c = C_v + kv_a a1 + kv_j j1
+    double p_a, p_j, cx_a, cx_j, cv_a, cv_j, kx_a, kx_j, kv_a, kv_j;
 };
+
+inline void fill_step_constants(StepArgs& a) {
+    const double h = a.dt, h2 = h * h, h3 = h2 * h;
+    a.p_a = 0.5 * h2;
+    a.p_j = h3 / 6.0;
+    a.cx_a = 0.35 * h2;
+    a.cx_j = 0.05 * h3;
+    a.cv_a = 0.5 * h;
+    a.cv_j = h2 / 12.0;
+    a.kx_a = 0.15 * h2;
+    a.kx_j = -h3 / 30.0;
+    a.kv_a = 0.5 * h;
+    a.kv_j = -h2 / 12.0;
+}
 
 // How a system of N bodies is spread over a warp: L lanes per system (odd, so the ring of lanes splits the
 // cross pairs evenly), B bodies per lane, L * B >= N (slots beyond N are massless far-away dummies).

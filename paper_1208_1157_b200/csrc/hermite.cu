@@ -32,7 +32,19 @@ ENS_SHAPE(2, 1, 2, true, 64, 1)
 ENS_SHAPE_T(3, 1, 3, ENS_H3_UNROLL, ENS_H3_THREADS, ENS_H3_MINB, ENS_H3_MAXT)
 ENS_SHAPE(4, 1, 4, false, 64, 1)
 ENS_SHAPE(5, 1, 5, false, 64, 1)
-ENS_SHAPE(6, 3, 2, false, 64, 1)
+#ifndef ENS_H6_L
+#define ENS_H6_L 3
+#define ENS_H6_B 2
+#endif
+#ifndef ENS_H6_THREADS
+#define ENS_H6_THREADS 64
+#define ENS_H6_MAXT 128
+#define ENS_H6_MINB 1
+#endif
+#ifndef ENS_H6_UNROLL
+#define ENS_H6_UNROLL false
+#endif
+ENS_SHAPE_T(6, ENS_H6_L, ENS_H6_B, ENS_H6_UNROLL, ENS_H6_THREADS, ENS_H6_MINB, ENS_H6_MAXT)
 ENS_SHAPE(7, 3, 3, false, 64, 1)
 ENS_SHAPE(8, 3, 3, false, 64, 1)
 ENS_SHAPE(9, 3, 3, false, 64, 1)
@@ -41,7 +53,16 @@ ENS_SHAPE(11, 3, 4, false, 64, 1)
 ENS_SHAPE(12, 3, 4, false, 64, 1)
 ENS_SHAPE(13, 5, 3, false, 64, 1)
 ENS_SHAPE(14, 5, 3, false, 64, 1)
-ENS_SHAPE(15, 5, 3, false, 64, 1)
+#ifndef ENS_H15_L
+#define ENS_H15_L 5
+#define ENS_H15_B 3
+#endif
+#ifndef ENS_H15_THREADS
+#define ENS_H15_THREADS 64
+#define ENS_H15_MAXT 128
+#define ENS_H15_MINB 1
+#endif
+ENS_SHAPE_T(15, ENS_H15_L, ENS_H15_B, false, ENS_H15_THREADS, ENS_H15_MINB, ENS_H15_MAXT)
 ENS_SHAPE(16, 5, 4, false, 64, 1)
 #undef ENS_SHAPE
 #undef ENS_SHAPE_T

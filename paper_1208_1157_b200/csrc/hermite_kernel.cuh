@@ -194,11 +194,8 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
     //   x_p = x + h v + h^2/2 a0 + h^3/6 j0          v_p = v + h a0 + h^2/2 j0
     //   C_x = x + h v + 7/20 h^2 a0 + 1/20 h^3 j0    C_v = v + h/2 a0 + 1/12 h^2 j0
     //   x_c = C_x + 3/20 h^2 a1 - 1/30 h^3 j1        v_c = C_v + h/2 a1 - 1/12 h^2 j1
+    // The ten coefficients come precomputed in StepArgs (constant bank operands of the DFMAs: no registers).
     const double h = p.dt;
-    const double h2 = h * h, h3 = h2 * h;
-    const double p_a = 0.5 * h2, p_j = h3 / 6.0;
-    const double cx_a = 0.35 * h2, cx_j = 0.05 * h3, cv_a = 0.5 * h, cv_j = h2 / 12.0;
-    const double kx_a = 0.15 * h2, kx_j = -h3 / 30.0, kv_a = 0.5 * h, kv_j = -h2 / 12.0;
     const bool fwd = h > 0.0;
 
     double Cx[B][3], Cv[B][3];
@@ -230,10 +227,10 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     const double tx = fma(h, V[b][c], X[b][c]);
-                    Cx[b][c] = fma(cx_j, j[b][c], fma(cx_a, a[b][c], tx));
-                    Cv[b][c] = fma(cv_j, j[b][c], fma(cv_a, a[b][c], V[b][c]));
-                    X[b][c] = fma(p_j, j[b][c], fma(p_a, a[b][c], tx));
-                    V[b][c] = fma(p_a, j[b][c], fma(h, a[b][c], V[b][c]));
+                    Cx[b][c] = fma(p.cx_j, j[b][c], fma(p.cx_a, a[b][c], tx));
+                    Cv[b][c] = fma(p.cv_j, j[b][c], fma(p.cv_a, a[b][c], V[b][c]));
+                    X[b][c] = fma(p.p_j, j[b][c], fma(p.p_a, a[b][c], tx));
+                    V[b][c] = fma(p.p_a, j[b][c], fma(h, a[b][c], V[b][c]));
                 }
         }
     };
@@ -242,8 +239,8 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
         for (int b = 0; b < B; ++b)
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                X[b][c] = fma(kx_j, j[b][c], fma(kx_a, a[b][c], Cx[b][c]));
-                V[b][c] = fma(kv_j, j[b][c], fma(kv_a, a[b][c], Cv[b][c]));
+                X[b][c] = fma(p.kx_j, j[b][c], fma(p.kx_a, a[b][c], Cx[b][c]));
+                V[b][c] = fma(p.kv_j, j[b][c], fma(p.kv_a, a[b][c], Cv[b][c]));
             }
     };
 
