@@ -171,9 +171,15 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3],
+                    help="Hermite workload (BASELINE.json configs index); 1 is the metric's, the others are for profiling")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--no-extras", action="store_true", help="skip the MVS / e2e / peak legs (profiling runs)")
     args = ap.parse_args()
+    global CFG, METRIC
+    if args.config != CFG:
+        CFG = args.config
+        METRIC = "hermite_fp64_system_steps_per_sec_" + W.CONFIGS[CFG].name.split("_", 1)[1]
     if args.impl == "reference":
         return run_reference(args)
     args.warmup = max(args.warmup, 3)
@@ -265,7 +271,7 @@ def main():
             k_ms = statistics.mean(kern_ms)
             peak_inst, peak_tf = nominal_fp64_peak(props.multi_processor_count, clocks.get("sm_max_mhz") or 1965.0)
             ach_tf = flops * n_sys * c.steps / (k_ms * 1e-3) / 1e12
-            roof = {"bound": "alu", "kernel": "hermite_kernel<3,1,3>", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+            roof = {"bound": "alu", "kernel": f"hermite_kernel<{n_body},{info['lanes_per_system']},{info['bodies_per_lane']}>", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
                     "frac": ach_tf / peak_tf, "traffic": None,
                     "peak_source": f"derived: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x "
                                    f"{clocks.get('sm_max_mhz') or 1965.0:.0f} MHz (DESIGN.md §8)",

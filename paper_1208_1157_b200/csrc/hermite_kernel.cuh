@@ -11,7 +11,7 @@
 //   * pairs across lanes: ring schedule.  At shift s = 1..(L-1)/2 lane l fetches the bodies of lane (l+s) mod L
 //     with warp shuffles, accumulates its own half of each pair in registers and the visitor's half (Newton's
 //     third law) in a temporary that is shuffled back to the owner.  No shared memory, no __syncthreads.
-// L = 1 (n_body <= 5) is "one system per thread" and contains no shuffle at all.
+// L = 1 (n_body <= 6) is "one system per thread" and contains no shuffle at all.
 //
 // The first evaluation of step k+1 is the evaluation of the post-step-k state, so its minimum pair distance IS
 // the close-approach monitor Alg. 1 places after step k: monitors cost no extra pair work, and a
@@ -68,6 +68,28 @@ __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const dou
         for (int c = 0; c < 3; ++c) a[b][c] = j[b][c] = 0.0;
     r2min = ~0ull;
 
+    // Cross-lane schedule (L > 1), written so that shuffle latency hides behind FP64 work of the same warp (a warp
+    // issues in order: an instruction that waits on a shuffle blocks everything behind it):
+    //   fetch(1) | in-lane pairs | for s = 1..H: { fetch(s+1) | B*B pairs of shift s | add returns of shift s-1 |
+    //   send returns of shift s } | add returns of shift H
+    constexpr int H = (L - 1) / 2;
+    double xv[2][B][3], vv[2][B][3], mv[2][B];  // visitors, double-buffered over the shifts
+    auto fetch = [&](int s, int buf) {
+        int ls = l + s;
+        if (ls >= L) ls -= L;
+        const int src = base + ls;  // whose bodies visit this lane at shift s
+#pragma unroll
+        for (int c = 0; c < B; ++c) {
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                xv[buf][c][q] = __shfl_sync(amask, x[c][q], src);
+                vv[buf][c][q] = __shfl_sync(amask, v[c][q], src);
+            }
+            mv[buf][c] = __shfl_sync(amask, m[c], src);
+        }
+    };
+    if constexpr (L > 1) fetch(1, 1);
+
     // pairs inside the lane.  Order: pairs among bodies 1.. first, pairs with local body 0 last, so that on lane 0
     // every planet receives the star's (largest) contribution last (for L = 1 this is exactly the
     // oracle's order: planets ascending, then the star).
@@ -82,36 +104,53 @@ __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const dou
     }
 
     if constexpr (L > 1) {
+        double ra[B][3], rj[B][3];  // the other half of MY bodies' pairs, computed by lane l - s
 #pragma unroll
-        for (int s = 1; s <= (L - 1) / 2; ++s) {
+        for (int s = 1; s <= H; ++s) {
+            const int buf = s & 1;
+            if (s < H) fetch(s + 1, buf ^ 1);
             int ls = l + s;
             if (ls >= L) ls -= L;
             int lr = l - s;
             if (lr < 0) lr += L;
-            const int src = base + ls;  // whose bodies visit this lane
-            const int ret = base + lr;  // which lane computed the other half of MY bodies' pairs at this shift
+            const int ret = base + lr;
+            double av[B][3], jv[B][3];
 #pragma unroll
             for (int c = 0; c < B; ++c) {
-                double xv[3], vv[3], av[3] = {0.0, 0.0, 0.0}, jv[3] = {0.0, 0.0, 0.0};
 #pragma unroll
-                for (int q = 0; q < 3; ++q) {
-                    xv[q] = __shfl_sync(amask, x[c][q], src);
-                    vv[q] = __shfl_sync(amask, v[c][q], src);
-                }
-                const double mv = __shfl_sync(amask, m[c], src);
+                for (int q = 0; q < 3; ++q) av[c][q] = jv[c][q] = 0.0;
                 const bool vvalid = !PADDED || (ls * B + c < N);
 #pragma unroll
                 for (int b = 0; b < B; ++b) {
-                    const double r2 = pair_acc_jerk(x[b], v[b], m[b], a[b], j[b], xv, vv, mv, av, jv);
+                    const double r2 = pair_acc_jerk(x[b], v[b], m[b], a[b], j[b], xv[buf][c], vv[buf][c], mv[buf][c],
+                                                    av[c], jv[c]);
                     min_bits(r2min, r2, vvalid && (!PADDED || (l * B + b < N)));
                 }
+            }
+            if (s > 1) {
+#pragma unroll
+                for (int c = 0; c < B; ++c)
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) {
+                        a[c][q] += ra[c][q];
+                        j[c][q] += rj[c][q];
+                    }
+            }
+#pragma unroll
+            for (int c = 0; c < B; ++c)
 #pragma unroll
                 for (int q = 0; q < 3; ++q) {
-                    a[c][q] += __shfl_sync(amask, av[q], ret);
-                    j[c][q] += __shfl_sync(amask, jv[q], ret);
+                    ra[c][q] = __shfl_sync(amask, av[c][q], ret);
+                    rj[c][q] = __shfl_sync(amask, jv[c][q], ret);
                 }
-            }
         }
+#pragma unroll
+        for (int c = 0; c < B; ++c)
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                a[c][q] += ra[c][q];
+                j[c][q] += rj[c][q];
+            }
     }
 }
 
