@@ -24,6 +24,21 @@ __device__ __forceinline__ double rsqrt_f64(double r2) {
     return fma(q, p, y0);
 }
 
+// FP64 reciprocal without the IEEE divide sequence: MUFU.RCP seed of the value rounded to FP32 (relative error
+// <= 2^-22), then y = y0 + y0 e (1 + e), e = 1 - x y0: remaining error e^3 < 2^-66 plus rounding (<= 1 ulp).
+// REFINE = false stops at y0 + y0 e (relative error 2^-44): enough for a Newton step, which is self-correcting.
+// Valid for |x| inside the FP32 normal range.
+template <bool REFINE>
+__device__ __forceinline__ double rcp_f64(double x) {
+    float s;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(__double2float_rn(x)));
+    const double y0 = (double)s;
+    const double e = fma(-x, y0, 1.0);
+    const double q = y0 * e;
+    if constexpr (REFINE) return fma(q, 1.0 + e, y0);
+    return y0 + q;
+}
+
 __device__ __forceinline__ void min_bits(u64& acc, double r2, bool valid = true) {
     // r2 >= 0 or NaN: unsigned order of the bit patterns is the numeric order and NaN sorts above +inf, so this
     // minimum runs on the integer ALU, not the FP64 pipe.

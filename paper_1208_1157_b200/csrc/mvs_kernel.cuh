@@ -24,33 +24,38 @@
 
 namespace ensd {
 
-// Stumpff functions c_n(z) = sum_k (-z)^k / (2k+n)!  (R-M3).  |z| is quartered until <= 0.1, the series is summed
-// there (8 terms: truncation < 1e-21 relative), and c_n(4z) is rebuilt from c_n(z) by the duplication formulas.
-// For the step sizes of the workloads (h << orbital period) z = beta X^2 is small and both loops run zero times.
-__device__ __forceinline__ void stumpff(double z, double& c0, double& c1, double& c2, double& c3) {
+// Stumpff functions c_n(z) = sum_k (-z)^k / (2k+n)!  (R-M3), series part: valid for |z| <= 0.1 (8 terms: truncation
+// < 1e-21 relative).  For the step sizes of the workloads (h << orbital period) z = beta X^2 is always in this range.
+__constant__ double kStumpff[16] = {
+    // descending powers of z, c2 / c3 interleaved: -1/16!, -1/17!, 1/14!, 1/15!, ..., 1/2!, 1/3!
+    -1.0 / 20922789888000.0, -1.0 / 355687428096000.0, 1.0 / 87178291200.0, 1.0 / 1307674368000.0,
+    -1.0 / 479001600.0,      -1.0 / 6227020800.0,      1.0 / 3628800.0,     1.0 / 39916800.0,
+    -1.0 / 40320.0,          -1.0 / 362880.0,          1.0 / 720.0,         1.0 / 5040.0,
+    -1.0 / 24.0,             -1.0 / 120.0,             0.5,                 1.0 / 6.0};
+
+__device__ __forceinline__ void stumpff_series(double z, double& c0, double& c1, double& c2, double& c3) {
+    // Horner in z; the coefficients are constant-bank operands of the DFMAs (no registers, no immediates to build)
+    double s2 = kStumpff[0], s3 = kStumpff[1];
+#pragma unroll
+    for (int k = 1; k < 8; ++k) {
+        s2 = fma(s2, z, kStumpff[2 * k]);
+        s3 = fma(s3, z, kStumpff[2 * k + 1]);
+    }
+    c2 = s2;
+    c3 = s3;
+    c1 = fma(-z, c3, 1.0);
+    c0 = fma(-z, c2, 1.0);
+}
+
+// General argument: |z| is quartered until <= 0.1, the series is summed there, and c_n(4z) is rebuilt from c_n(z) by
+// the duplication formulas.  Out of line: only steps of a sizeable fraction of an orbital period come here.
+__device__ __noinline__ void stumpff_general(double z, double& c0, double& c1, double& c2, double& c3) {
     int nq = 0;
     while (fabs(z) > 0.1) {
         z *= 0.25;
         ++nq;
     }
-    double s2 = -1.0 / 20922789888000.0;    // -1/16!
-    double s3 = -1.0 / 355687428096000.0;   // -1/17!
-    s2 = fma(s2, z, 1.0 / 87178291200.0);   //  1/14!
-    s3 = fma(s3, z, 1.0 / 1307674368000.0); //  1/15!
-    s2 = fma(s2, z, -1.0 / 479001600.0);    // -1/12!
-    s3 = fma(s3, z, -1.0 / 6227020800.0);   // -1/13!
-    s2 = fma(s2, z, 1.0 / 3628800.0);       //  1/10!
-    s3 = fma(s3, z, 1.0 / 39916800.0);      //  1/11!
-    s2 = fma(s2, z, -1.0 / 40320.0);        // -1/8!
-    s3 = fma(s3, z, -1.0 / 362880.0);       // -1/9!
-    s2 = fma(s2, z, 1.0 / 720.0);           //  1/6!
-    s3 = fma(s3, z, 1.0 / 5040.0);          //  1/7!
-    s2 = fma(s2, z, -1.0 / 24.0);           // -1/4!
-    s3 = fma(s3, z, -1.0 / 120.0);          // -1/5!
-    c2 = fma(s2, z, 0.5);                   //  1/2!
-    c3 = fma(s3, z, 1.0 / 6.0);             //  1/3!
-    c1 = fma(-z, c3, 1.0);
-    c0 = fma(-z, c2, 1.0);
+    stumpff_series(z, c0, c1, c2, c3);
     for (; nq > 0; --nq) {
         const double n3 = 0.25 * fma(c0, c3, c2);
         const double n2 = 0.5 * c1 * c1;
@@ -61,6 +66,13 @@ __device__ __forceinline__ void stumpff(double z, double& c0, double& c1, double
         c1 = n1;
         c0 = n0;
     }
+}
+
+__device__ __forceinline__ void stumpff(double z, double& c0, double& c1, double& c2, double& c3) {
+    if (fabs(z) <= 0.1)
+        stumpff_series(z, c0, c1, c2, c3);
+    else
+        stumpff_general(z, c0, c1, c2, c3);
 }
 
 struct KeplerG {
@@ -101,38 +113,84 @@ __device__ __noinline__ double kepler_bisect(double r0, double eta, double mu, d
     return 0.5 * (lo + hi);
 }
 
-// Advance (q, p) along the Kepler orbit about a fixed centre of gravitational parameter mu for time tau.
-__device__ __forceinline__ void kepler_drift(double (&q)[3], double (&p)[3], double mu, double tau) {
-    const double r0 = sqrt(fma(q[2], q[2], fma(q[1], q[1], q[0] * q[0])));
-    const double eta = fma(q[2], p[2], fma(q[1], p[1], q[0] * p[0]));
-    const double v2 = fma(p[2], p[2], fma(p[1], p[1], p[0] * p[0]));
-    const double beta = 2.0 * mu / r0 - v2;
-    double X = tau / r0;
-    bool ok = false;
-    for (int it = 0; it < 50; ++it) {
-        const KeplerG g = kepler_G(beta, X);
-        const double F = fma(r0, g.G1, fma(eta, g.G2, fma(mu, g.G3, -tau)));
-        const double dF = fma(r0, g.G0, fma(eta, g.G1, mu * g.G2));
-        const double dX = F / dF;
-        X -= dX;
-        if (!(fabs(dX) > 1e-15 * fabs(X))) {
-            ok = true;
-            break;
+// Kepler drift of the B planets of this lane about a fixed centre of gravitational parameter mu for time tau
+// (R-M3, R-M4).  The same root as the oracle's plain Newton iteration, reached with fewer evaluations of
+// the G functions and no IEEE divide:
+//   * the B planets are iterated together, so that B independent dependency chains are in flight (DFMA latency 8
+//     cycles against an issue interval of 2: one Kepler solve alone leaves the FP64 pipe mostly idle);
+//   * each iteration is Newton's step d1 = F / F' with Chebyshev's third-order correction d1 (1 + F F'' / (2 F'^2)),
+//     F' = r, F'' = eta G0 + (mu - beta r0) G1 (derivatives of the G functions: G0' = -beta G1, G_n' = G_{n-1});
+//     the correction is dropped when it is not small, which leaves Newton's step;
+//   * when every planet's step is below 1e-6 |X| the iteration has converged to far below rounding (the error after
+//     the step is of order |dX / X|^3), and the G functions at the final X follow from a second-order Taylor update
+//     with those same derivatives (neglected terms < 1e-18 relative) instead of one more Stumpff evaluation;
+//   * 1 / r0 comes from the reciprocal square root of |q|^2 and 1 / r from rcp_f64.
+// valid(b) = false leaves slot b untouched (massless dummy slots of padded shapes).
+template <int B, class Valid>
+__device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[B][3], double mu, double tau,
+                                                 Valid valid) {
+    double r0[B], ir0[B], eta[B], beta[B], X[B], d[B];
+    KeplerG g[B];
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+        const double r02 = fma(Q[b][2], Q[b][2], fma(Q[b][1], Q[b][1], Q[b][0] * Q[b][0]));
+        eta[b] = fma(Q[b][2], P[b][2], fma(Q[b][1], P[b][1], Q[b][0] * P[b][0]));
+        const double v2 = fma(P[b][2], P[b][2], fma(P[b][1], P[b][1], P[b][0] * P[b][0]));
+        ir0[b] = rsqrt_f64(r02);
+        r0[b] = r02 * ir0[b];
+        beta[b] = fma(2.0 * mu, ir0[b], -v2);
+        X[b] = tau * ir0[b];
+    }
+    bool done = false;
+    for (int it = 0; it < 50 && !done; ++it) {
+        done = true;
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            g[b] = kepler_G(beta[b], X[b]);
+            const double F = fma(r0[b], g[b].G1, fma(eta[b], g[b].G2, fma(mu, g[b].G3, -tau)));
+            const double r = fma(r0[b], g[b].G0, fma(eta[b], g[b].G1, mu * g[b].G2));
+            const double F2 = fma(eta[b], g[b].G0, fma(-beta[b], r0[b], mu) * g[b].G1);
+            const double ir = rcp_f64<false>(r);
+            const double d1 = F * ir;
+            double c = (0.5 * d1) * (F2 * ir);
+            c = fabs(c) < 0.1 ? c : 0.0;
+            const double dX = fma(d1, c, d1);
+            X[b] -= dX;
+            d[b] = -dX;
+            done = done && (fabs(dX) <= 1e-6 * fabs(X[b]));
         }
     }
-    if (!ok || !(fabs(X) <= DBL_MAX)) X = kepler_bisect(r0, eta, mu, beta, tau);
-    const KeplerG g = kepler_G(beta, X);
-    const double r = fma(r0, g.G0, fma(eta, g.G1, mu * g.G2));
-    const double f = 1.0 - mu * g.G2 / r0;
-    const double gg = fma(-mu, g.G3, tau);
-    const double fd = -mu * g.G1 / (r0 * r);
-    const double gd = 1.0 - mu * g.G2 / r;
 #pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        const double qn = fma(f, q[c], gg * p[c]);
-        const double pn = fma(fd, q[c], gd * p[c]);
-        q[c] = qn;
-        p[c] = pn;
+    for (int b = 0; b < B; ++b) {
+        if (!done || !(fabs(X[b]) <= DBL_MAX)) {  // not converged within the cap (or NaN): bisect, then G at the root
+            if (!(fabs(d[b]) <= 1e-6 * fabs(X[b]))) {
+                X[b] = kepler_bisect(r0[b], eta[b], mu, beta[b], tau);
+                g[b] = kepler_G(beta[b], X[b]);
+                d[b] = 0.0;
+            }
+        }
+        // G_n(X + d) to second order in d
+        const double hd = 0.5 * d[b], bg1 = beta[b] * g[b].G1, bg0 = beta[b] * g[b].G0;
+        const double G3 = fma(d[b], fma(hd, g[b].G1, g[b].G2), g[b].G3);
+        const double G2 = fma(d[b], fma(hd, g[b].G0, g[b].G1), g[b].G2);
+        const double G1 = fma(d[b], fma(-hd, bg1, g[b].G0), g[b].G1);
+        const double G0 = fma(-d[b], fma(hd, bg0, bg1), g[b].G0);
+        const double r = fma(r0[b], G0, fma(eta[b], G1, mu * G2));
+        const double ir = rcp_f64<true>(r);
+        const double mG2 = mu * G2;
+        const double f = fma(-mG2, ir0[b], 1.0);
+        const double gg = fma(-mu, G3, tau);
+        const double fd = -(mu * G1) * (ir0[b] * ir);
+        const double gd = fma(-mG2, ir, 1.0);
+        if (valid(b)) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double qn = fma(f, Q[b][c], gg * P[b][c]);
+                const double pn = fma(fd, Q[b][c], gd * P[b][c]);
+                Q[b][c] = qn;
+                P[b][c] = pn;
+            }
+        }
     }
 }
 
@@ -238,7 +296,7 @@ __global__ void __launch_bounds__(MAXT, MINB) mvs_kernel(View e, StepArgs p) {
 
     double Q[B][3], V[B][3], A[B][3], m[B];
     double Xcm[3] = {0.0, 0.0, 0.0}, Vcm[3] = {0.0, 0.0, 0.0};
-    double m0 = 1.0, Mtot = 1.0, t = 0.0;
+    double m0 = 1.0, im0 = 1.0, Mtot = 1.0, t = 0.0;
     int st = ENS_STOP_NONFINITE;
     bool active = false;
 #pragma unroll
@@ -271,6 +329,7 @@ __global__ void __launch_bounds__(MAXT, MINB) mvs_kernel(View e, StepArgs p) {
                 sv[c] = fma(mi, vi, sv[c]);
             }
         }
+        im0 = 1.0 / m0;  // one IEEE divide per launch; the step loop multiplies (<= 1 ulp from the oracle's s / m0)
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             Xcm[c] = sx[c] / Mtot;
@@ -315,7 +374,7 @@ __global__ void __launch_bounds__(MAXT, MINB) mvs_kernel(View e, StepArgs p) {
             eval_acc_planets<P, L, B>(Q, m, A, r2min, l, base, amask);
             mass_weighted_sum<L, B>(V, m, s, l, base, amask);
 #pragma unroll
-            for (int c = 0; c < 3; ++c) s[c] = s[c] / m0;
+            for (int c = 0; c < 3; ++c) s[c] = s[c] * im0;
         }
     }
 
@@ -335,9 +394,7 @@ __global__ void __launch_bounds__(MAXT, MINB) mvs_kernel(View e, StepArgs p) {
                 Xcm[c] = fma(hh, Vcm[c], Xcm[c]);
             }
             // 3: Kepler drift of every planet about mu = G m_0 (G = 1)
-#pragma unroll
-            for (int b = 0; b < B; ++b)
-                if (!PADDED || (l * B + b < P)) kepler_drift(Q[b], V[b], m0, h);
+            kepler_drift_all<B>(Q, V, m0, h, [&](int b) { return !PADDED || (l * B + b < P); });
             // 4: planet-planet accelerations at the new positions, half kick
             eval_acc_planets<P, L, B>(Q, m, A, r2min, l, base, amask);
 #pragma unroll
@@ -348,7 +405,7 @@ __global__ void __launch_bounds__(MAXT, MINB) mvs_kernel(View e, StepArgs p) {
             mass_weighted_sum<L, B>(V, m, s, l, base, amask);
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                s[c] = s[c] / m0;
+                s[c] = s[c] * im0;
                 const double sh = hh * s[c];
 #pragma unroll
                 for (int b = 0; b < B; ++b) Q[b][c] += sh;

@@ -104,7 +104,13 @@ def test_large_steps_eccentric_and_negative_dt():
         e.integrate(ens.MVS, -0.05, 400, t_end=-np.inf)
         r = e.get_state()
     assert rel_diff(f["pos"], pos).max() > 1e-2
-    assert rel_diff(r["pos"], pos).max() <= 1e-10 and np.abs(r["time"]).max() <= 1e-12
+    # the reversal defect is rounding noise amplified by each system's own sensitivity: judge it per system against
+    # the oracle's own forward-backward defect (R-M6, R-noise), 1e-11 where the oracle's is smaller than that
+    of = oracle.integrate(oracle.MVS, pos, vel, mass, dt=0.05, max_steps=400)
+    orv = oracle.integrate(oracle.MVS, of["pos"], of["vel"], mass, of["time"], dt=-0.05, max_steps=400, t_end=-np.inf)
+    d, dref = rel_diff(r["pos"], pos), rel_diff(orv["pos"], pos)
+    assert (d <= np.maximum(1e-11, 10 * dref)).all(), (d / np.maximum(1e-11, dref)).max()
+    assert np.median(d) <= 1e-12 and np.abs(r["time"]).max() <= 1e-12
 
 
 def test_test_particles_follow_kepler_orbits_exactly():
