@@ -272,7 +272,10 @@ def main():
             peak_inst, peak_tf = nominal_fp64_peak(props.multi_processor_count, clocks.get("sm_max_mhz") or 1965.0)
             ach_tf = flops * n_sys * c.steps / (k_ms * 1e-3) / 1e12
             roof = {"bound": "alu", "kernel": f"hermite_kernel<{n_body},{info['lanes_per_system']},{info['bodies_per_lane']}>", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                    "frac": ach_tf / peak_tf, "traffic": None,
+                    "frac": ach_tf / peak_tf,
+                    # ncu dram__bytes_read.sum + dram__bytes_write.sum of this kernel, one launch, config 1
+                    # (profiles/r1c_hermite_cfg1_ncu_full.txt); the store drains from L2 after the kernel ends
+                    "traffic": 24.7e6 if CFG == 1 else None,
                     "peak_source": f"derived: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x "
                                    f"{clocks.get('sm_max_mhz') or 1965.0:.0f} MHz (DESIGN.md §8)",
                     "kernel_ms": k_ms, "algorithmic_fp64_instr_per_system_step": instr,
@@ -317,21 +320,39 @@ def main():
                            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "passes": n_e2e,
                            "timing": "host wall clock around ens_set_state(HOST) + ens_integrate + ens_get_state(HOST) + "
                                      "ens_energy(HOST), pinned buffers"}
-            # second kernel: MVS on config 4 (own throughput; not part of the Hermite metric)
-            c4 = W.CONFIGS[4]
-            try:
-                p4, v4, m4 = (torch.from_numpy(x).cuda() for x in W.generate(4, offset=rank * c4.n_sys))
-                e4 = ens.Ensemble(c4.n_sys, c4.n_body)
-                ms4 = []
-                for _ in range(3):
-                    e4.set_state(p4, v4, m4, stream=stream)
-                    e4.integrate(ens.MVS, c4.dt, c4.steps, stream=stream)
-                    ms4.append(e4.last_kernel_ms())
-                line["mvs"] = {"workload": c4.name, "value": c4.n_sys * c4.steps / (min(ms4[1:]) * 1e-3),
-                               "unit": "system-steps/s", "kernel_ms": min(ms4[1:]), "regs": e4.info()["regs"]}
-                e4.close()
-            except ens.EnsError as ex:
-                line["mvs"] = {"unavailable": str(ex)}
+            # the other kernels of the path, each on its own BASELINE.json config at full size (kernel time only; not
+            # part of the metric): Hermite n_body = 6 and 15, and the second kernel, MVS on config 4
+            others = {}
+            for k in (2, 3, 4):
+                if k == CFG:
+                    continue
+                ck = W.CONFIGS[k]
+                try:
+                    pk, vk, mk = (torch.from_numpy(x).cuda() for x in W.generate(k, offset=rank * ck.n_sys))
+                    ek = ens.Ensemble(ck.n_sys, ck.n_body)
+                    ek.set_monitors(ck.r_close, ck.r_eject)
+                    msk = []
+                    for _ in range(3):
+                        ek.set_state(pk, vk, mk, stream=stream)
+                        ek.integrate(ck.integrator, ck.dt, ck.steps, stream=stream)
+                        msk.append(ek.last_kernel_ms())
+                    ik, tk = ek.info(), min(msk[1:])
+                    o = {"value": ck.n_sys * ck.steps / (tk * 1e-3), "unit": "system-steps/s", "kernel_ms": tk,
+                         "regs": ik["regs"], "lanes_per_system": ik["lanes_per_system"],
+                         "bodies_per_lane": ik["bodies_per_lane"], "blocks_per_sm": ik["blocks_per_sm"]}
+                    if ck.integrator == W.HERMITE:
+                        ins, _ = hermite_work(ck.n_body)
+                        o["issue_frac_nominal"] = o["value"] * ins / nominal_fp64_peak(
+                            torch.cuda.get_device_properties(local).multi_processor_count,
+                            clocks.get("sm_max_mhz") or 1965.0)[0]
+                    others[ck.name] = o
+                    ek.close()
+                    del pk, vk, mk
+                except ens.EnsError as ex:
+                    others[ck.name] = {"unavailable": str(ex)}
+            line["other_workloads"] = others
+            if W.CONFIGS[4].name in others:
+                line["mvs"] = dict(others[W.CONFIGS[4].name], workload=W.CONFIGS[4].name)
 
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         cb, _ = cpu_baseline()

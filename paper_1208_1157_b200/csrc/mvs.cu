@@ -7,38 +7,39 @@ namespace {
 
 // n_body -> lanes per system L (odd), planets per lane B, L * B >= n_body - 1 (the star is held by every lane).
 template <int N> struct MvsShape;
-#define ENS_MVS_SHAPE(N_, L_, B_, THREADS_, MINB_)                             \
+#define ENS_MVS_SHAPE(N_, L_, B_, THREADS_, MAXREG_)                           \
     template <> struct MvsShape<N_> {                                          \
-        static constexpr int L = L_, B = B_, THREADS = THREADS_, MINB = MINB_; \
+        static constexpr int L = L_, B = B_, THREADS = THREADS_, MAXREG = MAXREG_; \
     };
-//            N   L  B  threads minBlocks
-ENS_MVS_SHAPE(2, 1, 1, 128, 1)
-ENS_MVS_SHAPE(3, 1, 2, 128, 1)
-// config 4 (3 planets): 64-thread blocks, registers capped at 128 -> 16 warps per SM: 7.6 ms per 1000 steps against
-// 9.5 ms at 192 registers / 8 warps
+//            N   L  B  threads maxRegisters
+ENS_MVS_SHAPE(2, 1, 1, 128, 255)
+ENS_MVS_SHAPE(3, 1, 2, 128, 255)
+// config 4 (3 planets): tuned in DESIGN.md §8
 #ifndef ENS_M4_THREADS
 #define ENS_M4_THREADS 64
-#define ENS_M4_MINB 7
 #endif
-ENS_MVS_SHAPE(4, 1, 3, ENS_M4_THREADS, ENS_M4_MINB)
-ENS_MVS_SHAPE(5, 1, 4, 128, 1)
-ENS_MVS_SHAPE(6, 1, 5, 128, 1)
-ENS_MVS_SHAPE(7, 3, 2, 128, 1)
-ENS_MVS_SHAPE(8, 3, 3, 128, 1)
-ENS_MVS_SHAPE(9, 3, 3, 128, 1)
-ENS_MVS_SHAPE(10, 3, 3, 128, 1)
-ENS_MVS_SHAPE(11, 5, 2, 128, 1)
-ENS_MVS_SHAPE(12, 3, 4, 128, 1)
-ENS_MVS_SHAPE(13, 3, 4, 128, 1)
-ENS_MVS_SHAPE(14, 5, 3, 128, 1)
-ENS_MVS_SHAPE(15, 5, 3, 128, 1)
-ENS_MVS_SHAPE(16, 5, 3, 128, 1)
+#ifndef ENS_M4_MAXREG
+#define ENS_M4_MAXREG 168
+#endif
+ENS_MVS_SHAPE(4, 1, 3, ENS_M4_THREADS, ENS_M4_MAXREG)
+ENS_MVS_SHAPE(5, 1, 4, 128, 255)
+ENS_MVS_SHAPE(6, 1, 5, 128, 255)
+ENS_MVS_SHAPE(7, 3, 2, 128, 255)
+ENS_MVS_SHAPE(8, 3, 3, 128, 255)
+ENS_MVS_SHAPE(9, 3, 3, 128, 255)
+ENS_MVS_SHAPE(10, 3, 3, 128, 255)
+ENS_MVS_SHAPE(11, 5, 2, 128, 255)
+ENS_MVS_SHAPE(12, 3, 4, 128, 255)
+ENS_MVS_SHAPE(13, 3, 4, 128, 255)
+ENS_MVS_SHAPE(14, 5, 3, 128, 255)
+ENS_MVS_SHAPE(15, 5, 3, 128, 255)
+ENS_MVS_SHAPE(16, 5, 3, 128, 255)
 #undef ENS_MVS_SHAPE
 
 template <int N>
 constexpr auto kernel_ptr() {
     using S = MvsShape<N>;
-    return &mvs_kernel<N, S::L, S::B, S::THREADS, S::MINB>;
+    return &mvs_kernel<N, S::L, S::B, S::MAXREG>;
 }
 
 template <int N>

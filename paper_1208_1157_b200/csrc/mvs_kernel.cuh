@@ -47,48 +47,50 @@ __device__ __forceinline__ void stumpff_series(double z, double& c0, double& c1,
     c0 = fma(-z, c2, 1.0);
 }
 
+struct Stumpff {
+    double c0, c1, c2, c3;
+};
+
 // General argument: |z| is quartered until <= 0.1, the series is summed there, and c_n(4z) is rebuilt from c_n(z) by
-// the duplication formulas.  Out of line: only steps of a sizeable fraction of an orbital period come here.
-__device__ __noinline__ void stumpff_general(double z, double& c0, double& c1, double& c2, double& c3) {
+// the duplication formulas.  Out of line (returns in registers): only steps of a sizeable fraction of an orbital
+// period come here.
+__device__ __noinline__ Stumpff stumpff_general(double z) {
     int nq = 0;
     while (fabs(z) > 0.1) {
         z *= 0.25;
         ++nq;
     }
-    stumpff_series(z, c0, c1, c2, c3);
+    Stumpff c;
+    stumpff_series(z, c.c0, c.c1, c.c2, c.c3);
     for (; nq > 0; --nq) {
-        const double n3 = 0.25 * fma(c0, c3, c2);
-        const double n2 = 0.5 * c1 * c1;
-        const double n1 = c0 * c1;
-        const double n0 = fma(2.0 * c0, c0, -1.0);
-        c3 = n3;
-        c2 = n2;
-        c1 = n1;
-        c0 = n0;
+        const double n3 = 0.25 * fma(c.c0, c.c3, c.c2);
+        const double n2 = 0.5 * c.c1 * c.c1;
+        const double n1 = c.c0 * c.c1;
+        const double n0 = fma(2.0 * c.c0, c.c0, -1.0);
+        c.c3 = n3;
+        c.c2 = n2;
+        c.c1 = n1;
+        c.c0 = n0;
     }
-}
-
-__device__ __forceinline__ void stumpff(double z, double& c0, double& c1, double& c2, double& c3) {
-    if (fabs(z) <= 0.1)
-        stumpff_series(z, c0, c1, c2, c3);
-    else
-        stumpff_general(z, c0, c1, c2, c3);
+    return c;
 }
 
 struct KeplerG {
     double G0, G1, G2, G3;
 };
 
-__device__ __forceinline__ KeplerG kepler_G(double beta, double X) {
-    const double X2 = X * X;
-    double c0, c1, c2, c3;
-    stumpff(beta * X2, c0, c1, c2, c3);
+__device__ __forceinline__ KeplerG kepler_G_from(const Stumpff& c, double X, double X2) {
     KeplerG g;
-    g.G0 = c0;
-    g.G1 = X * c1;
-    g.G2 = X2 * c2;
-    g.G3 = (X2 * X) * c3;
+    g.G0 = c.c0;
+    g.G1 = X * c.c1;
+    g.G2 = X2 * c.c2;
+    g.G3 = (X2 * X) * c.c3;
     return g;
+}
+
+__device__ __forceinline__ KeplerG kepler_G(double beta, double X) {  // general argument (fallback path only)
+    const double X2 = X * X;
+    return kepler_G_from(stumpff_general(beta * X2), X, X2);
 }
 
 // Residual of the universal Kepler equation; monotone in X (its derivative is the radius r > 0).
@@ -113,18 +115,27 @@ __device__ __noinline__ double kepler_bisect(double r0, double eta, double mu, d
     return 0.5 * (lo + hi);
 }
 
+// |x| as the high word of its bit pattern (sign cleared): exponent and the top 20 mantissa bits.  Order-preserving
+// for finite values, NaN and inf sort at or above 0x7ff00000: threshold tests on the integer ALU instead of DSETP.
+__device__ __forceinline__ int abs_hi(double x) { return __double2hiint(x) & 0x7fffffff; }
+constexpr int kHi0p1 = 0x3fb99999;  // high word of 0.1 (0x3FB999999999999A), rounded down
+constexpr int kHiInf = 0x7ff00000;
+
 // Kepler drift of the B planets of this lane about a fixed centre of gravitational parameter mu for time tau
 // (R-M3, R-M4).  The same root as the oracle's plain Newton iteration, reached with fewer evaluations of
-// the G functions and no IEEE divide:
-//   * the B planets are iterated together, so that B independent dependency chains are in flight (DFMA latency 8
-//     cycles against an issue interval of 2: one Kepler solve alone leaves the FP64 pipe mostly idle);
+// the G functions, no IEEE divide, and straight-line code over the planets:
+//   * the B planets are iterated together, every stage written as a loop over b with no branch inside, so that B
+//     independent dependency chains are in flight (DFMA latency 8 cycles against an issue interval of 2: one Kepler
+//     solve alone leaves the FP64 pipe mostly idle);
 //   * each iteration is Newton's step d1 = F / F' with Chebyshev's third-order correction d1 (1 + F F'' / (2 F'^2)),
 //     F' = r, F'' = eta G0 + (mu - beta r0) G1 (derivatives of the G functions: G0' = -beta G1, G_n' = G_{n-1});
 //     the correction is dropped when it is not small, which leaves Newton's step;
 //   * when every planet's step is below 1e-6 |X| the iteration has converged to far below rounding (the error after
 //     the step is of order |dX / X|^3), and the G functions at the final X follow from a second-order Taylor update
 //     with those same derivatives (neglected terms < 1e-18 relative) instead of one more Stumpff evaluation;
-//   * 1 / r0 comes from the reciprocal square root of |q|^2 and 1 / r from rcp_f64.
+//   * 1 / r0 comes from the reciprocal square root of |q|^2 and 1 / r from rcp_f64;
+//   * Stumpff arguments beyond the series range (|z| > 0.1: steps of a sizeable fraction of a period) and lanes
+//     that fail to converge within the cap take out-of-line general paths.
 // valid(b) = false leaves slot b untouched (massless dummy slots of padded shapes).
 template <int B, class Valid>
 __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[B][3], double mu, double tau,
@@ -143,32 +154,52 @@ __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[
     }
     bool done = false;
     for (int it = 0; it < 50 && !done; ++it) {
-        done = true;
+        double X2[B], z[B];
+        Stumpff cs[B];
+        int zmax = 0;
 #pragma unroll
         for (int b = 0; b < B; ++b) {
-            g[b] = kepler_G(beta[b], X[b]);
+            X2[b] = X[b] * X[b];
+            z[b] = beta[b] * X2[b];
+            zmax = max(zmax, abs_hi(z[b]));
+        }
+        if (zmax < kHi0p1) {
+#pragma unroll
+            for (int b = 0; b < B; ++b) stumpff_series(z[b], cs[b].c0, cs[b].c1, cs[b].c2, cs[b].c3);
+        } else {
+#pragma unroll
+            for (int b = 0; b < B; ++b) cs[b] = stumpff_general(z[b]);
+        }
+        int conv = 1;
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            g[b] = kepler_G_from(cs[b], X[b], X2[b]);
             const double F = fma(r0[b], g[b].G1, fma(eta[b], g[b].G2, fma(mu, g[b].G3, -tau)));
             const double r = fma(r0[b], g[b].G0, fma(eta[b], g[b].G1, mu * g[b].G2));
             const double F2 = fma(eta[b], g[b].G0, fma(-beta[b], r0[b], mu) * g[b].G1);
             const double ir = rcp_f64<false>(r);
             const double d1 = F * ir;
             double c = (0.5 * d1) * (F2 * ir);
-            c = fabs(c) < 0.1 ? c : 0.0;
+            c = abs_hi(c) < kHi0p1 ? c : 0.0;
             const double dX = fma(d1, c, d1);
             X[b] -= dX;
             d[b] = -dX;
-            done = done && (fabs(dX) <= 1e-6 * fabs(X[b]));
+            conv &= (abs_hi(dX) <= abs_hi(1e-6 * X[b])) & (abs_hi(X[b]) < kHiInf);
         }
+        done = conv != 0;
     }
+    if (!done) {  // some planet of this lane did not converge within the cap (or went non-finite): bisect those
 #pragma unroll
-    for (int b = 0; b < B; ++b) {
-        if (!done || !(fabs(X[b]) <= DBL_MAX)) {  // not converged within the cap (or NaN): bisect, then G at the root
-            if (!(fabs(d[b]) <= 1e-6 * fabs(X[b]))) {
+        for (int b = 0; b < B; ++b) {
+            if (!((abs_hi(d[b]) <= abs_hi(1e-6 * X[b])) & (abs_hi(X[b]) < kHiInf))) {
                 X[b] = kepler_bisect(r0[b], eta[b], mu, beta[b], tau);
                 g[b] = kepler_G(beta[b], X[b]);
                 d[b] = 0.0;
             }
         }
+    }
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
         // G_n(X + d) to second order in d
         const double hd = 0.5 * d[b], bg1 = beta[b] * g[b].G1, bg0 = beta[b] * g[b].G0;
         const double G3 = fma(d[b], fma(hd, g[b].G1, g[b].G2), g[b].G3);
@@ -281,8 +312,10 @@ __device__ __forceinline__ void mass_weighted_sum(const double (&W)[B][3], const
     }
 }
 
-template <int N, int L, int B, int MAXT, int MINB>
-__global__ void __launch_bounds__(MAXT, MINB) mvs_kernel(View e, StepArgs p) {
+// MAXREG caps the registers per thread (and with them the resident warps per SM) directly: __launch_bounds__'s
+// minBlocks lets ptxas round down to a register count that spills.  Blocks must not exceed 65536 / MAXREG threads.
+template <int N, int L, int B, int MAXREG>
+__global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
     constexpr int P = N - 1;   // planets; body 0 is the star
     constexpr int S = 32 / L;  // systems per warp
     constexpr bool PADDED = (L * B != P);
