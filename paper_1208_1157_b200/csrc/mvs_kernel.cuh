@@ -152,8 +152,7 @@ __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[
         beta[b] = fma(2.0 * mu, ir0[b], -v2);
         X[b] = tau * ir0[b];
     }
-    bool done = false;
-    for (int it = 0; it < 50 && !done; ++it) {
+    auto iterate = [&]() -> bool {
         double X2[B], z[B];
         Stumpff cs[B];
         int zmax = 0;
@@ -186,8 +185,17 @@ __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[
             d[b] = -dX;
             conv &= (abs_hi(dX) <= abs_hi(1e-6 * X[b])) & (abs_hi(X[b]) < kHiInf);
         }
-        done = conv != 0;
-    }
+        return conv != 0;
+    };
+    // Two evaluations are always needed (the second confirms convergence, and is harmless if the first already
+    // had): straight-line code for them, a loop only for the rare third and later ones.
+#ifndef ENS_MVS_PEEL
+#define ENS_MVS_PEEL 2
+#endif
+    bool done = false;
+#pragma unroll
+    for (int it = 0; it < ENS_MVS_PEEL; ++it) done = iterate();
+    for (int it = ENS_MVS_PEEL; it < 50 && !done; ++it) done = iterate();
     if (!done) {  // some planet of this lane did not converge within the cap (or went non-finite): bisect those
 #pragma unroll
         for (int b = 0; b < B; ++b) {
@@ -450,20 +458,27 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
             // monitors on the post-step state (Alg. 1 execute(M); R11).  Planet-planet separations are
             // those of the acceleration evaluation: the drift shifts every planet alike.
             int f = 0;
-            double sq[3] = {0.0, 0.0, 0.0};
-            if (mon_eject) mass_weighted_sum<L, B>(Q, m, sq, l, base, amask);
-            double x0[3];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) x0[c] = Xcm[c] - sq[c] / Mtot;
             if (mon_close && r2min < p.rc2_bits) f |= 1;
-            if (mon_eject && dbits(fma(x0[2], x0[2], fma(x0[1], x0[1], x0[0] * x0[0]))) > p.re2_bits) f |= 2;
+            u64 q2max = 0ull, q2min = ~0ull;  // over this lane's planets: star-planet separation is |Q_i|
 #pragma unroll
             for (int b = 0; b < B; ++b) {
                 if (!PADDED || (l * B + b < P)) {
                     const u64 q2 = dbits(fma(Q[b][2], Q[b][2], fma(Q[b][1], Q[b][1], Q[b][0] * Q[b][0])));
-                    if (q2 > 0x7FEFFFFFFFFFFFFFull) f |= 4;  // +inf or NaN
-                    if (q2 < p.rc2_bits) f |= 1;             // star-planet separation is |Q_i|
-                    if (mon_eject) {
+                    q2max = q2 > q2max ? q2 : q2max;
+                    q2min = q2 < q2min ? q2 : q2min;
+                }
+            }
+            if (q2max > 0x7FEFFFFFFFFFFFFFull) f |= 4;  // +inf or NaN
+            if (q2min < p.rc2_bits) f |= 1;
+            if (mon_eject) {  // distances from the coordinate origin need the star's barycentric position
+                double sq[3], x0[3];
+                mass_weighted_sum<L, B>(Q, m, sq, l, base, amask);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) x0[c] = Xcm[c] - sq[c] / Mtot;
+                if (dbits(fma(x0[2], x0[2], fma(x0[1], x0[1], x0[0] * x0[0]))) > p.re2_bits) f |= 2;
+#pragma unroll
+                for (int b = 0; b < B; ++b) {
+                    if (!PADDED || (l * B + b < P)) {
                         const double xx = x0[0] + Q[b][0], yy = x0[1] + Q[b][1], zz = x0[2] + Q[b][2];
                         if (dbits(fma(zz, zz, fma(yy, yy, xx * xx))) > p.re2_bits) f |= 2;
                     }
