@@ -118,6 +118,10 @@ ENS_API int ens_fp64_peak(int64_t iters, double *lane_fma_per_s, void *stream);
  * FP64 refinement, P:L276 / R14), device pointers, n elements. */
 ENS_API int ens_test_rsqrt(const double *x, double *y, int64_t n, void *stream);
 
+/* Device function test hook: y[i] = the library's FP64 reciprocal of x[i] (float rcp seed + FP64 refinement; used
+ * by the MVS Kepler drift instead of the IEEE divide), device pointers, n elements. */
+ENS_API int ens_test_rcp(const double *x, double *y, int64_t n, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

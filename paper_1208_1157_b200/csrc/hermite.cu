@@ -132,6 +132,10 @@ __global__ void rsqrt_test_kernel(const double* x, double* y, int64_t n) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) y[i] = rsqrt_f64(x[i]);
 }
+__global__ void rcp_test_kernel(const double* x, double* y, int64_t n) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) y[i] = rcp_f64<true>(x[i]);
+}
 }  // namespace
 
 }  // namespace ensd
@@ -140,5 +144,12 @@ extern "C" ENS_API int ens_test_rsqrt(const double* x, double* y, int64_t n, voi
     if (!x || !y || n < 0) return ENS_EINVAL;
     if (n == 0) return ENS_OK;
     ensd::rsqrt_test_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(x, y, n);
+    return cudaGetLastError() == cudaSuccess ? ENS_OK : ENS_ECUDA;
+}
+
+extern "C" ENS_API int ens_test_rcp(const double* x, double* y, int64_t n, void* stream) {
+    if (!x || !y || n < 0) return ENS_EINVAL;
+    if (n == 0) return ENS_OK;
+    ensd::rcp_test_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(x, y, n);
     return cudaGetLastError() == cudaSuccess ? ENS_OK : ENS_ECUDA;
 }

@@ -23,6 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libens.so")
 SYMBOLS = (
     "ens_create", "ens_destroy", "ens_set_state", "ens_set_monitors", "ens_integrate", "ens_get_state",
     "ens_energy", "ens_strerror", "ens_get_info", "ens_last_kernel_ms", "ens_fp64_peak", "ens_test_rsqrt",
+    "ens_test_rcp",
 )
 _lib = None
 
@@ -57,6 +58,7 @@ def lib() -> ctypes.CDLL:
         L.ens_last_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
         L.ens_fp64_peak.argtypes = [i64, ctypes.POINTER(cd), vp]
         L.ens_test_rsqrt.argtypes = [vp, vp, i64, vp]
+        L.ens_test_rcp.argtypes = [vp, vp, i64, vp]
         for name in SYMBOLS:
             if name != "ens_strerror":
                 getattr(L, name).restype = ci
@@ -206,6 +208,12 @@ def fp64_peak(iters: int = 200000, stream=None) -> float:
 def rsqrt_probe(x: torch.Tensor) -> torch.Tensor:
     y = torch.empty_like(x)
     _check(lib().ens_test_rsqrt(x.data_ptr(), y.data_ptr(), x.numel(), _stream_ptr(None)), "ens_test_rsqrt")
+    return y
+
+
+def rcp_probe(x: torch.Tensor) -> torch.Tensor:
+    y = torch.empty_like(x)
+    _check(lib().ens_test_rcp(x.data_ptr(), y.data_ptr(), x.numel(), _stream_ptr(None)), "ens_test_rcp")
     return y
 
 

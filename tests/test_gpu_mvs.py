@@ -149,3 +149,17 @@ def test_monitors_time_stop_and_sticky_status():
         g2 = e.get_state()
         stopped = g["status"] >= ens.STOP_CLOSE
         assert (g2["pos"][stopped] == g["pos"][stopped]).all() and (g2["nsteps"][~stopped] == g["nsteps"][~stopped] + 5).all()
+
+
+def test_rcp_within_one_ulp():
+    """The MVS kernel's divide-free reciprocal (float rcp seed + cubic FP64 refinement) is within 1 ulp of the
+    correctly rounded 1/x over the radii it sees and near the ends of its documented domain, both signs."""
+    import torch
+    rng = np.random.default_rng(6)
+    x = np.concatenate([10.0 ** rng.uniform(-4, 4, 400000), 10.0 ** rng.uniform(-36, 36, 100000),
+                        -(10.0 ** rng.uniform(-4, 4, 1000)), np.array([1.0, 2.0, 3.0, 0.1, 7.0, 1e-3])])
+    y = ens.rcp_probe(torch.from_numpy(x).cuda()).cpu().numpy()
+    ref = 1.0 / x.astype(np.longdouble)
+    err = np.abs((y.astype(np.longdouble) - ref) / np.spacing(np.abs(ref).astype(np.float64))).astype(np.float64)
+    print(f"rcp: max error {err.max():.3f} ulp, mean {err.mean():.3f}")
+    assert err.max() <= 1.0
