@@ -25,7 +25,7 @@ _lock = threading.Lock()
 _lib = None
 
 ACTIVE, DONE_TIME, DONE_STEPS, STOP_CLOSE, STOP_EJECT, STOP_NONFINITE = range(6)
-HERMITE, MVS = 0, 1
+HERMITE, MVS, HERMITE_ADAPTIVE = 0, 1, 2  # for HERMITE_ADAPTIVE `dt` is the step size scale tau of Eq. 5
 DOUBLE, LONG_DOUBLE = 0, 1
 
 CXXFLAGS = ["-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-std=c++17"]
@@ -52,6 +52,7 @@ def _load():
         lib.orc_acc_jerk.argtypes = [ci, d, d, d, d, d, ci]
         lib.orc_hermite_step.argtypes = [ci, d, d, d, cd, ci, ci]
         lib.orc_integrate.argtypes = [ci, cl, ci, d, d, d, d, i32, i64, cd, cd, cl, cd, cd, ci, ci]
+        lib.orc_adaptive_dt.argtypes = [ci, d, d, d, cd, d, ci]
         lib.orc_energy.argtypes = [cl, ci, d, d, d, d, d, ci]
         lib.orc_stumpff.argtypes = [cd, d, ci]
         lib.orc_kepler_drift.argtypes = [d, d, cd, cd, ci, ctypes.POINTER(ci)]
@@ -91,6 +92,16 @@ def hermite_step(x, v, m, h, n_corr=2, prec=DOUBLE):
     rc = _load().orc_hermite_step(m.shape[0], _p(x), _p(v), _p(m), float(h), int(n_corr), prec)
     assert rc == 0
     return x, v
+
+
+def adaptive_dt(x, v, m, tau, prec=DOUBLE):
+    """Eq. 5: the step the adaptive Hermite integrator takes from state (x, v) of one system."""
+    x, v, m = _f64(x), _f64(v), _f64(m)
+    out = np.zeros(1)
+    rc = _load().orc_adaptive_dt(m.shape[0], _p(x), _p(v), _p(m), float(tau), _p(out), prec)
+    if rc:
+        raise ValueError("orc_adaptive_dt: bad arguments")
+    return float(out[0])
 
 
 def integrate(integrator, pos, vel, mass, time=None, *, dt, t_end=np.inf, max_steps, r_close=0.0, r_eject=np.inf,

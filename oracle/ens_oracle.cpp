@@ -113,6 +113,26 @@ void hermite_step(int n, R* x, R* v, const R* m, R h, int n_corr = 2) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Adaptive time step, Eq. 5:  dt = tau [ sum_i |j_i0|^2 / |a_i0|^2 ]^(-1/2),  i over ALL bodies of the
+// system ("i indexes a body in the system", the star included: reading R-A1), a_i0 and j_i0 evaluated at the
+// beginning of the step ("uses only the values at the beginning of the time step").  tau carries the
+// sign of the integration direction.  A body with |a|^2 = 0 (no other mass in the system) contributes nothing
+// (reading R-A2).  The step itself is hermite_step with this dt (same three evaluations, R6).
+// ---------------------------------------------------------------------------------------------------
+template <class R>
+R hermite_adaptive_dt(int n, const R* x, const R* v, const R* m, R tau) {
+    std::vector<R> a(3 * n), j(3 * n);
+    eval_acc_jerk(n, x, v, m, a.data(), j.data());
+    R sum = 0;
+    for (int i = 0; i < n; ++i) {
+        const R a2 = a[3 * i] * a[3 * i] + a[3 * i + 1] * a[3 * i + 1] + a[3 * i + 2] * a[3 * i + 2];
+        const R j2 = j[3 * i] * j[3 * i] + j[3 * i + 1] * j[3 * i + 1] + j[3 * i + 2] * j[3 * i + 2];
+        if (a2 > R(0)) sum += j2 / a2;
+    }
+    return tau / std::sqrt(sum);
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Monitors (Alg. 1 `execute(M)` after `advance(P)`; thresholds from BASELINE.json;
 // reading R11).  Evaluated on the post-step state only.  Order: non-finite, close approach, ejection.
 // ---------------------------------------------------------------------------------------------------
@@ -379,15 +399,20 @@ void run_system(int integrator, int n, double* pos, double* vel, const double* m
         if (!time_left(dt, (double)t, t_end)) { st = ST_DONE_TIME; break; }
         if (k >= max_steps) { st = ST_DONE_STEPS; break; }
         const R* xmon;
+        R hs = h;  // the step actually taken (t += hs below)
         if (integrator == 0) {
             hermite_step(n, x.data(), v.data(), m.data(), h, n_corr);
+            xmon = x.data();
+        } else if (integrator == 2) {  // adaptive Hermite: dt is the step size scale tau of Eq. 5
+            hs = hermite_adaptive_dt(n, x.data(), v.data(), m.data(), h);
+            hermite_step(n, x.data(), v.data(), m.data(), hs, n_corr);
             xmon = x.data();
         } else {
             mvs_step(s, m.data(), h);
             from_dh<R>(s, m.data(), xm.data(), nullptr);
             xmon = xm.data();
         }
-        t += h;
+        t += hs;
         ++k;
         const int mon = monitors(n, xmon, r_close, r_eject);
         if (mon != ST_ACTIVE) { st = mon; break; }
@@ -431,12 +456,12 @@ int orc_hermite_step(int n, double* x, double* v, const double* m, double h, int
     return 0;
 }
 
-// integrator: 0 = Hermite, 1 = MVS.  status/nsteps/time are in-out ([n_sys]); status STOP_* is sticky.
+// integrator: 0 = Hermite (fixed step dt), 1 = MVS, 2 = adaptive Hermite (dt = tau of Eq. 5).  status/nsteps/time are in-out ([n_sys]); status STOP_* is sticky.
 int orc_integrate(int integrator, int64_t n_sys, int n, double* pos, double* vel, const double* mass, double* time,
                   int32_t* status, int64_t* nsteps, double dt, double t_end, int64_t max_steps, double r_close,
                   double r_eject, int prec, int nthreads) {
     if (n_sys < 0 || n < 2 || !pos || !vel || !mass || !time || !status || !nsteps) return -1;
-    if (!(dt != 0) || !std::isfinite(dt) || max_steps < 0 || (integrator != 0 && integrator != 1)) return -1;
+    if (!(dt != 0) || !std::isfinite(dt) || max_steps < 0 || (integrator < 0 || integrator > 2)) return -1;
     if (nthreads < 1) nthreads = 1;
 #pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads)
     for (int64_t s = 0; s < n_sys; ++s) {
@@ -447,6 +472,18 @@ int orc_integrate(int integrator, int64_t n_sys, int n, double* pos, double* vel
             run_system<double>(integrator, n, p, w, mm, time + s, status + s, nsteps + s, dt, t_end, max_steps, r_close, r_eject, 2);
         else
             run_system<long double>(integrator, n, p, w, mm, time + s, status + s, nsteps + s, dt, t_end, max_steps, r_close, r_eject, 2);
+    }
+    return 0;
+}
+
+// dt of Eq. 5 for one system (test hook)
+int orc_adaptive_dt(int n, const double* x, const double* v, const double* m, double tau, double* dt, int prec) {
+    if (n < 2 || !x || !v || !m || !dt) return -1;
+    if (prec == 0) {
+        *dt = hermite_adaptive_dt<double>(n, x, v, m, tau);
+    } else {
+        std::vector<long double> X(x, x + 3 * n), V(v, v + 3 * n), M(m, m + n);
+        *dt = (double)hermite_adaptive_dt<long double>(n, X.data(), V.data(), M.data(), (long double)tau);
     }
     return 0;
 }
