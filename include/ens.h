@@ -38,7 +38,7 @@ extern "C" {
 typedef struct ens ens_t; /* opaque */
 
 enum { ENS_OK = 0, ENS_EINVAL = -1, ENS_ENOMEM = -2, ENS_ECUDA = -3, ENS_ESTATE = -4, ENS_EUNSUPPORTED = -5 };
-enum { ENS_HERMITE = 0, ENS_MVS = 1 };
+enum { ENS_HERMITE = 0, ENS_MVS = 1, ENS_HERMITE_ADAPTIVE = 2 };
 enum { ENS_HOST = 0, ENS_DEVICE = 1 };
 /* per-system status (Alg. 1 "state").  DONE_* become ACTIVE again at the next ens_integrate;
  * STOP_* are sticky until ens_set_state. */
@@ -79,7 +79,10 @@ ENS_API int ens_set_monitors(ens_t *e, double r_close, double r_eject);
  * (dt < 0) for pure step-count control.  integrator: ENS_HERMITE = predictor + 2 corrector iterations with 3
  * acceleration-and-jerk evaluations per step (Alg. 2; R3-R6); ENS_MVS = democratic-heliocentric
  * half-drift / half-kick / Kepler drift / half-kick / half-drift (R-M1..R-M7), which needs body 0
- * to dominate the mass.
+ * to dominate the mass; ENS_HERMITE_ADAPTIVE = the same Hermite step with the time step recomputed at the start of
+ * every step from Eq. 5, step = dt [ sum_i |j_i|^2 / |a_i|^2 ]^(-1/2) over all bodies of the system
+ * (R-A1, R-A2): here `dt` is the dimensionless step size scale tau (its sign gives the direction), every system
+ * takes its own steps, and `time` advances by the step actually taken.
  * EINVAL: NULL handle, unknown integrator, dt == 0 or non-finite, NaN t_end, max_steps < 0.
  * ESTATE: no state was set.  ECUDA: launch failed. */
 ENS_API int ens_integrate(ens_t *e, int integrator, double dt, double t_end, int64_t max_steps, void *stream);

@@ -165,7 +165,7 @@ struct ens {
     // device staging (AoS) for host-space calls, allocated on first use
     double* stage;        // [n_sys * n_body * 7] : pos | vel | mass
     double* stage_small;  // [n_sys * 4] : time / E | L   (also int32 status, int64 nsteps reuse)
-    ensd::KernelInfo hermite, mvs;
+    ensd::KernelInfo hermite, hermite_adaptive, mvs;
     int threads_override;
     int64_t last_blocks;
     const void* last_fn;
@@ -236,7 +236,8 @@ int ens_create(int64_t n_sys, int n_body, ens_t** out) {
         ens_destroy(e);
         return rc;
     }
-    e->hermite = ensd::hermite_kernel_for(n_body);
+    e->hermite = ensd::hermite_kernel_for(n_body, false);
+    e->hermite_adaptive = ensd::hermite_kernel_for(n_body, true);
     e->mvs = ensd::mvs_kernel_for(n_body);
     const char* env = getenv("ENS_THREADS");
     e->threads_override = env ? atoi(env) : 0;
@@ -306,7 +307,7 @@ int ens_set_state(ens_t* e, const double* pos, const double* vel, const double* 
 }
 
 int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max_steps, void* stream) {
-    if (!e || (integrator != ENS_HERMITE && integrator != ENS_MVS)) return ENS_EINVAL;
+    if (!e || (integrator != ENS_HERMITE && integrator != ENS_MVS && integrator != ENS_HERMITE_ADAPTIVE)) return ENS_EINVAL;
     if (!(dt != 0.0) || !std::isfinite(dt) || std::isnan(t_end) || max_steps < 0) return ENS_EINVAL;
     if (!e->have_state) return ENS_ESTATE;
     cudaStream_t s = (cudaStream_t)stream;
@@ -320,12 +321,15 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
     memcpy(&a.rc2_bits, &rc2, 8);
     memcpy(&a.re2_bits, &re2, 8);
     ensd::fill_step_constants(a);
-    const ensd::KernelInfo& ki = integrator == ENS_HERMITE ? e->hermite : e->mvs;
+    const ensd::KernelInfo& ki = integrator == ENS_HERMITE            ? e->hermite
+                                 : integrator == ENS_HERMITE_ADAPTIVE ? e->hermite_adaptive
+                                                                      : e->mvs;
     if (!ki.fn) return ENS_EUNSUPPORTED;
     const int threads = e->threads_override ? e->threads_override : ki.threads;
     CU(cudaEventRecord(e->ev0, s));
-    cudaError_t err = integrator == ENS_HERMITE ? ensd::launch_hermite(e->v, a, threads, s, &e->last_blocks)
-                                                : ensd::launch_mvs(e->v, a, threads, s, &e->last_blocks);
+    cudaError_t err = integrator == ENS_MVS
+                          ? ensd::launch_mvs(e->v, a, threads, s, &e->last_blocks)
+                          : ensd::launch_hermite(e->v, a, integrator == ENS_HERMITE_ADAPTIVE, threads, s, &e->last_blocks);
     if (err != cudaSuccess) return cuda_fail(err, "ens_integrate launch");
     CU(cudaEventRecord(e->ev1, s));
     e->last_fn = ki.fn;
@@ -394,7 +398,9 @@ int ens_energy(const ens_t* e, double* E, double* L, int memspace, void* stream)
 
 int ens_get_info(const ens_t* e, int64_t out[8]) {
     if (!e || !out) return ENS_EINVAL;
-    const ensd::KernelInfo& ki = (e->last_fn && e->last_fn == e->mvs.fn) ? e->mvs : e->hermite;
+    const ensd::KernelInfo& ki = (e->last_fn && e->last_fn == e->mvs.fn)                ? e->mvs
+                                 : (e->last_fn && e->last_fn == e->hermite_adaptive.fn) ? e->hermite_adaptive
+                                                                                        : e->hermite;
     const int threads = e->threads_override ? e->threads_override : ki.threads;
     out[0] = e->v.n_pad;
     out[1] = ki.shape.L;

@@ -65,8 +65,9 @@ struct KernelInfo {
 };
 
 // hermite_*.cu / mvs.cu
-KernelInfo hermite_kernel_for(int n_body);
-cudaError_t launch_hermite(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out);
+KernelInfo hermite_kernel_for(int n_body, bool adaptive);
+cudaError_t launch_hermite(const View& v, const StepArgs& a, bool adaptive, int threads, cudaStream_t s,
+                           int64_t* blocks_out);
 KernelInfo mvs_kernel_for(int n_body);
 cudaError_t launch_mvs(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out);
 

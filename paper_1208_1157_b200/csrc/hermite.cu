@@ -69,24 +69,24 @@ ENS_SHAPE(16, 5, 4, false, 64, 1)
 #undef ENS_SHAPE
 #undef ENS_SHAPE_T
 
-template <int N>
+template <int N, bool ADAPT>
 constexpr auto kernel_ptr() {
     using S = ShapeOf<N>;
-    return &hermite_kernel<N, S::L, S::B, S::UNROLL, S::MAXT, S::MINB>;
+    return &hermite_kernel<N, S::L, S::B, S::UNROLL, S::MAXT, S::MINB, ADAPT>;
 }
 
-template <int N>
+template <int N, bool ADAPT>
 KernelInfo info_of() {
     using S = ShapeOf<N>;
     KernelInfo k;
-    k.fn = (const void*)kernel_ptr<N>();
+    k.fn = (const void*)kernel_ptr<N, ADAPT>();
     k.shape.L = S::L;
     k.shape.B = S::B;
     k.threads = S::THREADS;
     return k;
 }
 
-template <int N>
+template <int N, bool ADAPT>
 cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
     using S = ShapeOf<N>;
     if (threads > S::MAXT) threads = S::MAXT;  // __launch_bounds__ of the kernel
@@ -95,7 +95,7 @@ cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t
     const int wpb = threads / 32;
     const int64_t blocks = (warps + wpb - 1) / wpb;
     if (blocks_out) *blocks_out = blocks;
-    kernel_ptr<N>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
+    kernel_ptr<N, ADAPT>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
     return cudaGetLastError();
 }
 
@@ -103,10 +103,10 @@ cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t
 
 #define ENS_FOR_EACH_N(X) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
 
-KernelInfo hermite_kernel_for(int n_body) {
+KernelInfo hermite_kernel_for(int n_body, bool adaptive) {
     switch (n_body) {
 #define X(N_) \
-    case N_: return info_of<N_>();
+    case N_: return adaptive ? info_of<N_, true>() : info_of<N_, false>();
         ENS_FOR_EACH_N(X)
 #undef X
     }
@@ -117,10 +117,12 @@ KernelInfo hermite_kernel_for(int n_body) {
     return none;
 }
 
-cudaError_t launch_hermite(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
+cudaError_t launch_hermite(const View& v, const StepArgs& a, bool adaptive, int threads, cudaStream_t s,
+                           int64_t* blocks_out) {
     switch (v.n_body) {
 #define X(N_) \
-    case N_: return launch_n<N_>(v, a, threads, s, blocks_out);
+    case N_:  \
+        return adaptive ? launch_n<N_, true>(v, a, threads, s, blocks_out) : launch_n<N_, false>(v, a, threads, s, blocks_out);
         ENS_FOR_EACH_N(X)
 #undef X
     }

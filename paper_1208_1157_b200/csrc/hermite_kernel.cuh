@@ -154,6 +154,35 @@ __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const dou
     }
 }
 
+// Adaptive time step, Eq. 5: dt = tau [ sum_i |j_i|^2 / |a_i|^2 ]^(-1/2) over ALL bodies of the system
+// (R-A1), from the acceleration and jerk at the beginning of the step; bodies that feel no acceleration are left out
+// (R-A2).  Every lane of the system gathers the per-lane partial sums in the same (lane) order, so all of them take
+// bit-identical steps.  Reciprocal and reciprocal square root come from the FP32 seeds + FP64 refinement (<= 1 ulp)
+// inside the FP32 range, from the IEEE sequences outside it.
+template <int N, int L, int B>
+__device__ __forceinline__ double adaptive_dt(const double (&a)[B][3], const double (&j)[B][3], double tau, int l,
+                                              int base, unsigned amask) {
+    constexpr bool PADDED = (L * B != N);
+    double part = 0.0;
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+        const double a2 = fma(a[b][2], a[b][2], fma(a[b][1], a[b][1], a[b][0] * a[b][0]));
+        const double j2 = fma(j[b][2], j[b][2], fma(j[b][1], j[b][1], j[b][0] * j[b][0]));
+        double ia2 = rcp_f64<true>(a2);
+        if (!(a2 > 1e-30 && a2 < 1e30)) ia2 = a2 > 0.0 ? 1.0 / a2 : 0.0;
+        if (!PADDED || (l * B + b < N)) part = fma(j2, ia2, part);
+    }
+    double sum = part;
+    if constexpr (L > 1) {
+        sum = __shfl_sync(amask, part, base);
+#pragma unroll
+        for (int i = 1; i < L; ++i) sum += __shfl_sync(amask, part, base + i);
+    }
+    double y = rsqrt_f64(sum);
+    if (!(sum > 1e-30 && sum < 1e30)) y = 1.0 / sqrt(sum);
+    return tau * y;
+}
+
 // bits: 1 = close approach, 2 = ejection, 4 = non-finite position; OR-reduced over the lanes of the system.
 template <int N, int L, int B>
 __device__ __forceinline__ int monitor_flags(const double (&x)[B][3], u64 r2min, const StepArgs& p, int l, int base,
@@ -185,7 +214,9 @@ __device__ __forceinline__ int monitor_flags(const double (&x)[B][3], u64 r2min,
 // UNROLL = true: the three evaluations of a step are three inlined copies (straight-line step, best for small
 // pair counts); false: one copy of the evaluation inside a 3-phase loop (keeps large-n kernels inside the
 // instruction cache and the live register set at x, v, C_x, C_v, a, j).
-template <int N, int L, int B, bool UNROLL, int MAXT, int MINB>
+// ADAPT = true: the adaptive-step integrator (Eq. 5): p.dt is the step size scale tau, the step h and the ten
+// coefficients are per system and per step (registers) instead of launch constants.
+template <int N, int L, int B, bool UNROLL, int MAXT, int MINB, bool ADAPT = false>
 __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p) {
     constexpr int S = 32 / L;  // systems per warp
     constexpr bool PADDED = (L * B != N);
@@ -234,8 +265,8 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
     //   C_x = x + h v + 7/20 h^2 a0 + 1/20 h^3 j0    C_v = v + h/2 a0 + 1/12 h^2 j0
     //   x_c = C_x + 3/20 h^2 a1 - 1/30 h^3 j1        v_c = C_v + h/2 a1 - 1/12 h^2 j1
     // The ten coefficients come precomputed in StepArgs (constant bank operands of the DFMAs: no registers).
-    const double h = p.dt;
-    const bool fwd = h > 0.0;
+    double h = p.dt;  // the step taken; ADAPT: recomputed from (a0, j0) at the start of every step
+    const bool fwd = p.dt > 0.0;
 
     double Cx[B][3], Cv[B][3];
     double a[B][3], j[B][3];
@@ -260,26 +291,48 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 active = false;
             }
         }
+        // lanes that just stopped take no part in the shuffles below: re-vote (every lane of amask is here)
+        unsigned am2 = amask;
+        if constexpr (ADAPT && L > 1) am2 = __ballot_sync(amask, active);
         if (active) {
+            double p_a = p.p_a, p_j = p.p_j, cx_a = p.cx_a, cx_j = p.cx_j, cv_a = p.cv_a, cv_j = p.cv_j;
+            if constexpr (ADAPT) {
+                h = adaptive_dt<N, L, B>(a, j, p.dt, l, base, am2);
+                const double h2 = h * h, h3 = h2 * h;
+                p_a = 0.5 * h2;
+                p_j = (1.0 / 6.0) * h3;
+                cx_a = 0.35 * h2;
+                cx_j = 0.05 * h3;
+                cv_a = 0.5 * h;
+                cv_j = (1.0 / 12.0) * h2;
+            }
 #pragma unroll
             for (int b = 0; b < B; ++b)
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     const double tx = fma(h, V[b][c], X[b][c]);
-                    Cx[b][c] = fma(p.cx_j, j[b][c], fma(p.cx_a, a[b][c], tx));
-                    Cv[b][c] = fma(p.cv_j, j[b][c], fma(p.cv_a, a[b][c], V[b][c]));
-                    X[b][c] = fma(p.p_j, j[b][c], fma(p.p_a, a[b][c], tx));
-                    V[b][c] = fma(p.p_a, j[b][c], fma(h, a[b][c], V[b][c]));
+                    Cx[b][c] = fma(cx_j, j[b][c], fma(cx_a, a[b][c], tx));
+                    Cv[b][c] = fma(cv_j, j[b][c], fma(cv_a, a[b][c], V[b][c]));
+                    X[b][c] = fma(p_j, j[b][c], fma(p_a, a[b][c], tx));
+                    V[b][c] = fma(p_a, j[b][c], fma(h, a[b][c], V[b][c]));
                 }
         }
     };
     auto correct = [&]() {
+        double kx_a = p.kx_a, kx_j = p.kx_j, kv_a = p.kv_a, kv_j = p.kv_j;
+        if constexpr (ADAPT) {  // rebuilt from h each time: one live register pair instead of four
+            const double h2 = h * h;
+            kx_a = 0.15 * h2;
+            kx_j = (-1.0 / 30.0) * (h2 * h);
+            kv_a = 0.5 * h;
+            kv_j = (-1.0 / 12.0) * h2;
+        }
 #pragma unroll
         for (int b = 0; b < B; ++b)
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
-                X[b][c] = fma(p.kx_j, j[b][c], fma(p.kx_a, a[b][c], Cx[b][c]));
-                V[b][c] = fma(p.kv_j, j[b][c], fma(p.kv_a, a[b][c], Cv[b][c]));
+                X[b][c] = fma(kx_j, j[b][c], fma(kx_a, a[b][c], Cx[b][c]));
+                V[b][c] = fma(kv_j, j[b][c], fma(kv_a, a[b][c], Cv[b][c]));
             }
     };
 
