@@ -166,6 +166,7 @@ struct ens {
     double* stage;        // [n_sys * n_body * 7] : pos | vel | mass
     double* stage_small;  // [n_sys * 4] : time / E | L   (also int32 status, int64 nsteps reuse)
     ensd::KernelInfo hermite, hermite_adaptive, mvs;
+    unsigned long long* counter;  // work counter of the adaptive kernels
     int threads_override;
     int64_t last_blocks;
     const void* last_fn;
@@ -229,6 +230,7 @@ int ens_create(int64_t n_sys, int n_body, ens_t** out) {
     alloc((void**)&e->v.time, sizeof(double) * np);
     alloc((void**)&e->v.status, sizeof(int32_t) * np);
     alloc((void**)&e->v.nsteps, sizeof(int64_t) * np);
+    alloc((void**)&e->counter, sizeof(unsigned long long));
     if (err == cudaSuccess) err = cudaEventCreate(&e->ev0);
     if (err == cudaSuccess) err = cudaEventCreate(&e->ev1);
     if (err != cudaSuccess) {
@@ -255,6 +257,7 @@ int ens_destroy(ens_t* e) {
     cudaFree(e->v.time);
     cudaFree(e->v.status);
     cudaFree(e->v.nsteps);
+    cudaFree(e->counter);
     cudaFree(e->stage);
     cudaFree(e->stage_small);
     if (e->ev0) cudaEventDestroy(e->ev0);
@@ -321,6 +324,8 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
     memcpy(&a.rc2_bits, &rc2, 8);
     memcpy(&a.re2_bits, &re2, 8);
     ensd::fill_step_constants(a);
+    a.counter = e->counter;
+    if (integrator == ENS_HERMITE_ADAPTIVE) CU(cudaMemsetAsync(e->counter, 0, sizeof(unsigned long long), s));
     const ensd::KernelInfo& ki = integrator == ENS_HERMITE            ? e->hermite
                                  : integrator == ENS_HERMITE_ADAPTIVE ? e->hermite_adaptive
                                                                       : e->mvs;

@@ -36,6 +36,7 @@ struct StepArgs {
     //   C_x = x + h v + cx_a a0 + cx_j j0            C_v = v + cv_a a0 + cv_j j0
     //   x_c = C_x + kx_a a1 + kx_j j1                v_c = C_v + kv_a a1 + kv_j j1
     double p_a, p_j, cx_a, cx_j, cv_a, cv_j, kx_a, kx_j, kv_a, kv_j;
+    unsigned long long* counter;  // adaptive kernels: next system index to hand out (zeroed before the launch)
 };
 
 inline void fill_step_constants(StepArgs& a) {

@@ -93,7 +93,17 @@ cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t
     const int64_t sys_per_warp = 32 / S::L;
     const int64_t warps = (v.n_sys + sys_per_warp - 1) / sys_per_warp;
     const int wpb = threads / 32;
-    const int64_t blocks = (warps + wpb - 1) / wpb;
+    int64_t blocks = (warps + wpb - 1) / wpb;
+    if constexpr (ADAPT) {  // persistent grid: what the device holds at once; lane groups pull systems from a.counter
+        int dev = 0, sms = 0, per_sm = 0;
+        cudaError_t err = cudaGetDevice(&dev);
+        if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (err == cudaSuccess)
+            err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel_ptr<N, ADAPT>(), threads, 0);
+        if (err != cudaSuccess) return err;
+        const int64_t resident = (int64_t)sms * (per_sm > 0 ? per_sm : 1);
+        if (blocks > resident) blocks = resident;
+    }
     if (blocks_out) *blocks_out = blocks;
     kernel_ptr<N, ADAPT>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
     return cudaGetLastError();

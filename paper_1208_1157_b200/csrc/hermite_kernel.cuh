@@ -225,26 +225,26 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
     const int sl = lane / L;
     const int l = lane - sl * L;
     const int base = sl * L;
-    const int64_t sys = warp * S + sl;
-    const bool live = (sl < S) && (sys < e.n_sys);
+    // Fixed step: system (warp * S + sl) for the whole launch.  ADAPT: a persistent grid; every group of L lanes pulls
+    // system indices from a device counter and pulls the next one when its system finishes (systems take different
+    // numbers of steps: a finished system must not leave its lanes idle until the slowest of the warp is done).
+    int64_t sys = warp * S + sl;
 
     double X[B][3], V[B][3], m[B];
     double t = 0.0;
     int st = ENS_STOP_NONFINITE;
-    bool active = false;
-#pragma unroll
-    for (int b = 0; b < B; ++b) {
-        // dummy slot (padded shapes only): massless, at rest, far from everything and from each other
-        const int gid = l * B + b;
-        X[b][0] = 1.0e8 * (double)(gid + 1);
-        X[b][1] = X[b][2] = 0.0;
-        V[b][0] = V[b][1] = V[b][2] = 0.0;
-        m[b] = 0.0;
-    }
-    if (live) {
+    bool active = false, writeback = false;
+    int64_t k = 0;
+
+    auto load_system = [&]() {  // sys -> registers; sets active / writeback
 #pragma unroll
         for (int b = 0; b < B; ++b) {
             const int gid = l * B + b;
+            // dummy slot (padded shapes only): massless, at rest, far from everything and from each other
+            X[b][0] = 1.0e8 * (double)(gid + 1);
+            X[b][1] = X[b][2] = 0.0;
+            V[b][0] = V[b][1] = V[b][2] = 0.0;
+            m[b] = 0.0;
             if (!PADDED || gid < N) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -256,9 +256,62 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
         }
         t = e.time[sys];
         st = e.status[sys];
+        k = 0;
         active = st < ENS_STOP_CLOSE;  // STOP_* are sticky; DONE_* run again
+        writeback = active;
+    };
+    auto store_system = [&]() {  // registers -> sys (only systems that were advanced)
+        if (writeback) {
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                const int gid = l * B + b;
+                if (!PADDED || gid < N) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        e.pos[(int64_t)(gid * 3 + c) * e.n_pad + sys] = X[b][c];
+                        e.vel[(int64_t)(gid * 3 + c) * e.n_pad + sys] = V[b][c];
+                    }
+                }
+            }
+            if (l == 0) {
+                e.time[sys] = t;
+                e.status[sys] = st;
+                e.nsteps[sys] += k;
+            }
+        }
+        writeback = false;
+    };
+
+    bool exhausted = !(sl < S);  // ADAPT: this lane group will pull no more systems
+    if constexpr (!ADAPT) {
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            X[b][0] = 1.0e8 * (double)(l * B + b + 1);
+            X[b][1] = X[b][2] = 0.0;
+            V[b][0] = V[b][1] = V[b][2] = 0.0;
+            m[b] = 0.0;
+        }
+        if ((sl < S) && (sys < e.n_sys)) load_system();
     }
-    const bool writeback = active;
+    // ADAPT only; called with the whole warp converged, at step boundaries: groups without a running system store
+    // the one they finished and pull the next index
+    auto refill = [&]() -> bool {
+        const bool want = !active && !exhausted;
+        const unsigned rmask = __ballot_sync(0xffffffffu, want);
+        if (want) {
+            store_system();
+            unsigned long long idx = 0;
+            if (l == 0) idx = atomicAdd(p.counter, 1ull);
+            if constexpr (L > 1) idx = __shfl_sync(rmask, idx, base);
+            if ((int64_t)idx < e.n_sys) {
+                sys = (int64_t)idx;
+                load_system();
+            } else {
+                exhausted = true;
+            }
+        }
+        return __ballot_sync(0xffffffffu, !exhausted) != 0;  // somebody may still be running or pulling
+    };
 
     // Eq. 3 / Eq. 4 with the step-size powers folded in (algebraically the oracle's formulas):
     //   x_p = x + h v + h^2/2 a0 + h^3/6 j0          v_p = v + h a0 + h^2/2 j0
@@ -271,13 +324,13 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
     double Cx[B][3], Cv[B][3];
     double a[B][3], j[B][3];
     u64 r2min;
-    int64_t k = 0;
 
     // phase 0 of the loop below; returns with `active` updated.  X, V hold the accepted state.
     auto accept_and_predict = [&](unsigned amask) {
-        if (k > 0) {  // monitors act on post-step states only (Alg. 1: advance, then execute(M))
+        {  // monitors act on post-step states only (Alg. 1: advance, then execute(M)).  Every active lane takes part
+           // in the flag reduction (with refilled systems k differs between the systems of a warp).
             const int f = monitor_flags<N, L, B>(X, r2min, p, l, base, amask);
-            if (f) {
+            if (k > 0 && f) {
                 st = (f & 4) ? ENS_STOP_NONFINITE : (f & 1) ? ENS_STOP_CLOSE : ENS_STOP_EJECT;
                 active = false;
             }
@@ -338,8 +391,14 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
 
     if constexpr (UNROLL) {
         while (true) {
+            if constexpr (ADAPT) {
+                if (!refill()) break;
+            }
             const unsigned amask = __ballot_sync(0xffffffffu, active);
-            if (amask == 0) break;
+            if (amask == 0) {
+                if constexpr (ADAPT) continue;
+                break;
+            }
             if (active) {
                 eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
                 accept_and_predict(amask);
@@ -354,47 +413,35 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
             }
         }
     } else {
-        int phase = 0;
+        int phase = 0;  // warp-uniform: 0 = accept + predict, 1 and 2 = corrector iterations
         while (true) {
+            if constexpr (ADAPT) {
+                if (phase == 0 && !refill()) break;
+            }
             const unsigned amask = __ballot_sync(0xffffffffu, active);
-            if (amask == 0) break;
+            if (amask == 0) {
+                if constexpr (ADAPT) {
+                    phase = 0;
+                    continue;
+                }
+                break;
+            }
             if (active) {
                 eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
                 if (phase == 0) {
                     accept_and_predict(amask);
-                    phase = 1;
                 } else {
                     correct();
                     if (phase == 2) {
                         t += h;
                         ++k;
-                        phase = 0;
-                    } else {
-                        phase = 2;
                     }
                 }
             }
+            phase = phase == 2 ? 0 : phase + 1;
         }
     }
-
-    if (writeback) {
-#pragma unroll
-        for (int b = 0; b < B; ++b) {
-            const int gid = l * B + b;
-            if (!PADDED || gid < N) {
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    e.pos[(int64_t)(gid * 3 + c) * e.n_pad + sys] = X[b][c];
-                    e.vel[(int64_t)(gid * 3 + c) * e.n_pad + sys] = V[b][c];
-                }
-            }
-        }
-        if (l == 0) {
-            e.time[sys] = t;
-            e.status[sys] = st;
-            e.nsteps[sys] += k;
-        }
-    }
+    store_system();
 }
 
 }  // namespace ensd
