@@ -274,7 +274,7 @@ def main():
             roof = {"bound": "alu", "kernel": f"hermite_kernel<{n_body},{info['lanes_per_system']},{info['bodies_per_lane']}>", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
                     "frac": ach_tf / peak_tf,
                     # ncu dram__bytes_read.sum + dram__bytes_write.sum of this kernel, one launch, config 1
-                    # (profiles/r1c_hermite_cfg1_ncu_full.txt); the store drains from L2 after the kernel ends
+                    # (profiles/r1g_hermite_cfg1_ncu_full.txt); the store drains from L2 after the kernel ends
                     "traffic": 24.7e6 if CFG == 1 else None,
                     "peak_source": f"derived: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x "
                                    f"{clocks.get('sm_max_mhz') or 1965.0:.0f} MHz (DESIGN.md §8)",
