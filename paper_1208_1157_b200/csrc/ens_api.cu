@@ -167,6 +167,7 @@ struct ens {
     double* stage_small;  // [n_sys * 4] : time / E | L   (also int32 status, int64 nsteps reuse)
     ensd::KernelInfo hermite, hermite_adaptive, mvs;
     unsigned long long* counter;  // work counter of the adaptive kernels
+    ensd::OrderBuffers order;     // hand-out order of the adaptive kernels (allocated on first use)
     int threads_override;
     int64_t last_blocks;
     const void* last_fn;
@@ -258,6 +259,7 @@ int ens_destroy(ens_t* e) {
     cudaFree(e->v.status);
     cudaFree(e->v.nsteps);
     cudaFree(e->counter);
+    ensd::adaptive_order_free(e->order);
     cudaFree(e->stage);
     cudaFree(e->stage_small);
     if (e->ev0) cudaEventDestroy(e->ev0);
@@ -325,7 +327,15 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
     memcpy(&a.re2_bits, &re2, 8);
     ensd::fill_step_constants(a);
     a.counter = e->counter;
-    if (integrator == ENS_HERMITE_ADAPTIVE) CU(cudaMemsetAsync(e->counter, 0, sizeof(unsigned long long), s));
+    a.order = nullptr;
+    if (integrator == ENS_HERMITE_ADAPTIVE) {
+        CU(cudaMemsetAsync(e->counter, 0, sizeof(unsigned long long), s));
+        if (!getenv("ENS_ADAPTIVE_UNORDERED")) {  // (the switch exists for the measurement in DESIGN.md §8)
+            CU(ensd::adaptive_order(e->v, t_end, e->order, s));
+            a.order = e->order.idx_out;
+            e->launches += 1;  // the key kernel (the sort is cub's)
+        }
+    }
     const ensd::KernelInfo& ki = integrator == ENS_HERMITE            ? e->hermite
                                  : integrator == ENS_HERMITE_ADAPTIVE ? e->hermite_adaptive
                                                                       : e->mvs;

@@ -37,6 +37,7 @@ struct StepArgs {
     //   x_c = C_x + kx_a a1 + kx_j j1                v_c = C_v + kv_a a1 + kv_j j1
     double p_a, p_j, cx_a, cx_j, cv_a, cv_j, kx_a, kx_j, kv_a, kv_j;
     unsigned long long* counter;  // adaptive kernels: next system index to hand out (zeroed before the launch)
+    const int32_t* order;         // adaptive kernels: hand-out order (longest expected run first), or nullptr
 };
 
 inline void fill_step_constants(StepArgs& a) {
@@ -64,6 +65,16 @@ struct KernelInfo {
     Shape shape;
     int threads;  // threads per block
 };
+
+// adaptive_order.cu: order[] = system indices sorted by decreasing expected number of adaptive steps
+struct OrderBuffers {
+    float *key_in = nullptr, *key_out = nullptr;
+    int32_t *idx_in = nullptr, *idx_out = nullptr;  // idx_out is the order
+    void* tmp = nullptr;
+    size_t tmp_bytes = 0;
+};
+cudaError_t adaptive_order(const View& v, double t_end, OrderBuffers& ob, cudaStream_t s);
+void adaptive_order_free(OrderBuffers& ob);
 
 // hermite_*.cu / mvs.cu
 KernelInfo hermite_kernel_for(int n_body, bool adaptive);

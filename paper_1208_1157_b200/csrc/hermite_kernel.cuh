@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
             if (l == 0) idx = atomicAdd(p.counter, 1ull);
             if constexpr (L > 1) idx = __shfl_sync(rmask, idx, base);
             if ((int64_t)idx < e.n_sys) {
-                sys = (int64_t)idx;
+                sys = p.order ? (int64_t)p.order[idx] : (int64_t)idx;  // longest expected run first (adaptive_order.cu)
                 load_system();
             } else {
                 exhausted = true;
