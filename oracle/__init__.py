@@ -25,7 +25,8 @@ _lock = threading.Lock()
 _lib = None
 
 ACTIVE, DONE_TIME, DONE_STEPS, STOP_CLOSE, STOP_EJECT, STOP_NONFINITE = range(6)
-HERMITE, MVS, HERMITE_ADAPTIVE = 0, 1, 2  # for HERMITE_ADAPTIVE `dt` is the step size scale tau of Eq. 5
+HERMITE, MVS, HERMITE_ADAPTIVE, HERMITE_CARRY = 0, 1, 2, 3
+# HERMITE_ADAPTIVE: `dt` is the step size scale tau of Eq. 5.  HERMITE_CARRY: Alg. 2 as printed, 2 evaluations per step.
 DOUBLE, LONG_DOUBLE = 0, 1
 
 CXXFLAGS = ["-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-std=c++17"]

@@ -113,6 +113,37 @@ void hermite_step(int n, R* x, R* v, const R* m, R h, int n_corr = 2) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Alg. 2 exactly as printed: TWO evaluations per step.  a^(0), j^(0) are inputs of the step, and the
+// loop leaves a^(2), j^(2) (evaluated at the iterate x^(2), v^(2), i.e. before the last correction) behind; the
+// next step takes them as its a^(0), j^(0) (reading R6-alt: "carry").  Coefficients and bases as in hermite_step
+// (R3-R5).  a0, j0: in = values for this step, out = values for the next one.
+// ---------------------------------------------------------------------------------------------------
+template <class R>
+void hermite_step_carry(int n, R* x, R* v, const R* m, R h, R* a0, R* j0) {
+    const int d = 3 * n;
+    std::vector<R> a1(d), j1(d), xp(d), vp(d), xc(d), vc(d);
+    for (int q = 0; q < d; ++q) {
+        xp[q] = x[q] + v[q] * h + a0[q] * (h * h) / R(2) + j0[q] * (h * h * h) / R(6);
+        vp[q] = v[q] + a0[q] * h + j0[q] * (h * h) / R(2);
+        xc[q] = xp[q];
+        vc[q] = vp[q];
+    }
+    for (int it = 0; it < 2; ++it) {
+        eval_acc_jerk(n, xc.data(), vc.data(), m, a1.data(), j1.data());
+        for (int q = 0; q < d; ++q) {
+            xc[q] = xp[q] - (R(3) / R(20)) * (a0[q] - a1[q]) * (h * h) - (R(1) / R(60)) * (R(7) * j0[q] + R(2) * j1[q]) * (h * h * h);
+            vc[q] = vp[q] - (R(1) / R(2)) * (a0[q] - a1[q]) * h - (R(1) / R(12)) * (R(5) * j0[q] + j1[q]) * (h * h);
+        }
+    }
+    for (int q = 0; q < d; ++q) {
+        x[q] = xc[q];
+        v[q] = vc[q];
+        a0[q] = a1[q];
+        j0[q] = j1[q];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Adaptive time step, Eq. 5:  dt = tau [ sum_i |j_i0|^2 / |a_i0|^2 ]^(-1/2),  i over ALL bodies of the
 // system ("i indexes a body in the system", the star included: reading R-A1), a_i0 and j_i0 evaluated at the
 // beginning of the step ("uses only the values at the beginning of the time step").  tau carries the
@@ -390,7 +421,9 @@ void run_system(int integrator, int n, double* pos, double* vel, const double* m
     int st = ST_ACTIVE;
     int64_t k = 0;
     DH<R> s;
-    std::vector<R> xm(3 * n);
+    std::vector<R> xm(3 * n), ca(3 * n), cj(3 * n);
+    if (integrator == 3)  // carried (a, j): evaluated once at the state the call starts from
+        eval_acc_jerk(n, x.data(), v.data(), m.data(), ca.data(), cj.data());
     if (integrator == 1) {
         to_dh(n, x.data(), v.data(), m.data(), s);
         eval_acc_planets(n, s.Q.data(), m.data(), s.A.data());  // prepare(P)
@@ -402,6 +435,9 @@ void run_system(int integrator, int n, double* pos, double* vel, const double* m
         R hs = h;  // the step actually taken (t += hs below)
         if (integrator == 0) {
             hermite_step(n, x.data(), v.data(), m.data(), h, n_corr);
+            xmon = x.data();
+        } else if (integrator == 3) {  // Alg. 2 as printed: 2 evaluations per step, (a, j) carried
+            hermite_step_carry(n, x.data(), v.data(), m.data(), h, ca.data(), cj.data());
             xmon = x.data();
         } else if (integrator == 2) {  // adaptive Hermite: dt is the step size scale tau of Eq. 5
             hs = hermite_adaptive_dt(n, x.data(), v.data(), m.data(), h);
@@ -456,12 +492,13 @@ int orc_hermite_step(int n, double* x, double* v, const double* m, double h, int
     return 0;
 }
 
-// integrator: 0 = Hermite (fixed step dt), 1 = MVS, 2 = adaptive Hermite (dt = tau of Eq. 5).  status/nsteps/time are in-out ([n_sys]); status STOP_* is sticky.
+// integrator: 0 = Hermite (fixed step dt), 1 = MVS, 2 = adaptive Hermite (dt = tau of Eq. 5),
+// 3 = Hermite with 2 evaluations per step (Alg. 2 as printed; a, j carried from step to step).  status/nsteps/time are in-out ([n_sys]); status STOP_* is sticky.
 int orc_integrate(int integrator, int64_t n_sys, int n, double* pos, double* vel, const double* mass, double* time,
                   int32_t* status, int64_t* nsteps, double dt, double t_end, int64_t max_steps, double r_close,
                   double r_eject, int prec, int nthreads) {
     if (n_sys < 0 || n < 2 || !pos || !vel || !mass || !time || !status || !nsteps) return -1;
-    if (!(dt != 0) || !std::isfinite(dt) || max_steps < 0 || (integrator < 0 || integrator > 2)) return -1;
+    if (!(dt != 0) || !std::isfinite(dt) || max_steps < 0 || (integrator < 0 || integrator > 3)) return -1;
     if (nthreads < 1) nthreads = 1;
 #pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads)
     for (int64_t s = 0; s < n_sys; ++s) {
