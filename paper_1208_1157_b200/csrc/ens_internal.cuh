@@ -77,8 +77,8 @@ cudaError_t adaptive_order(const View& v, double t_end, OrderBuffers& ob, cudaSt
 void adaptive_order_free(OrderBuffers& ob);
 
 // hermite_*.cu / mvs.cu
-KernelInfo hermite_kernel_for(int n_body, bool adaptive);
-cudaError_t launch_hermite(const View& v, const StepArgs& a, bool adaptive, int threads, cudaStream_t s,
+KernelInfo hermite_kernel_for(int n_body, int mode);  // mode: 0 fixed step, 1 adaptive, 2 carried a/j
+cudaError_t launch_hermite(const View& v, const StepArgs& a, int mode, int threads, cudaStream_t s,
                            int64_t* blocks_out);
 KernelInfo mvs_kernel_for(int n_body);
 cudaError_t launch_mvs(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out);

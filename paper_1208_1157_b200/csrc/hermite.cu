@@ -69,24 +69,25 @@ ENS_SHAPE(16, 5, 4, false, 64, 1)
 #undef ENS_SHAPE
 #undef ENS_SHAPE_T
 
-template <int N, bool ADAPT>
+// MODE: 0 = fixed step (3 evaluations), 1 = adaptive step, 2 = fixed step with carried a, j (2 evaluations)
+template <int N, int MODE>
 constexpr auto kernel_ptr() {
     using S = ShapeOf<N>;
-    return &hermite_kernel<N, S::L, S::B, S::UNROLL, S::MAXT, S::MINB, ADAPT>;
+    return &hermite_kernel<N, S::L, S::B, S::UNROLL, S::MAXT, S::MINB, MODE == 1, MODE == 2>;
 }
 
-template <int N, bool ADAPT>
+template <int N, int MODE>
 KernelInfo info_of() {
     using S = ShapeOf<N>;
     KernelInfo k;
-    k.fn = (const void*)kernel_ptr<N, ADAPT>();
+    k.fn = (const void*)kernel_ptr<N, MODE>();
     k.shape.L = S::L;
     k.shape.B = S::B;
     k.threads = S::THREADS;
     return k;
 }
 
-template <int N, bool ADAPT>
+template <int N, int MODE>
 cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
     using S = ShapeOf<N>;
     if (threads > S::MAXT) threads = S::MAXT;  // __launch_bounds__ of the kernel
@@ -94,18 +95,18 @@ cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t
     const int64_t warps = (v.n_sys + sys_per_warp - 1) / sys_per_warp;
     const int wpb = threads / 32;
     int64_t blocks = (warps + wpb - 1) / wpb;
-    if constexpr (ADAPT) {  // persistent grid: what the device holds at once; lane groups pull systems from a.counter
+    if constexpr (MODE == 1) {  // persistent grid: what the device holds at once; lane groups pull systems from a.counter
         int dev = 0, sms = 0, per_sm = 0;
         cudaError_t err = cudaGetDevice(&dev);
         if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (err == cudaSuccess)
-            err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel_ptr<N, ADAPT>(), threads, 0);
+            err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel_ptr<N, MODE>(), threads, 0);
         if (err != cudaSuccess) return err;
         const int64_t resident = (int64_t)sms * (per_sm > 0 ? per_sm : 1);
         if (blocks > resident) blocks = resident;
     }
     if (blocks_out) *blocks_out = blocks;
-    kernel_ptr<N, ADAPT>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
+    kernel_ptr<N, MODE>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
     return cudaGetLastError();
 }
 
@@ -113,10 +114,10 @@ cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t
 
 #define ENS_FOR_EACH_N(X) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
 
-KernelInfo hermite_kernel_for(int n_body, bool adaptive) {
+KernelInfo hermite_kernel_for(int n_body, int mode) {
     switch (n_body) {
 #define X(N_) \
-    case N_: return adaptive ? info_of<N_, true>() : info_of<N_, false>();
+    case N_: return mode == 1 ? info_of<N_, 1>() : mode == 2 ? info_of<N_, 2>() : info_of<N_, 0>();
         ENS_FOR_EACH_N(X)
 #undef X
     }
@@ -127,12 +128,14 @@ KernelInfo hermite_kernel_for(int n_body, bool adaptive) {
     return none;
 }
 
-cudaError_t launch_hermite(const View& v, const StepArgs& a, bool adaptive, int threads, cudaStream_t s,
+cudaError_t launch_hermite(const View& v, const StepArgs& a, int mode, int threads, cudaStream_t s,
                            int64_t* blocks_out) {
     switch (v.n_body) {
 #define X(N_) \
     case N_:  \
-        return adaptive ? launch_n<N_, true>(v, a, threads, s, blocks_out) : launch_n<N_, false>(v, a, threads, s, blocks_out);
+        return mode == 1   ? launch_n<N_, 1>(v, a, threads, s, blocks_out) \
+               : mode == 2 ? launch_n<N_, 2>(v, a, threads, s, blocks_out) \
+                           : launch_n<N_, 0>(v, a, threads, s, blocks_out);
         ENS_FOR_EACH_N(X)
 #undef X
     }

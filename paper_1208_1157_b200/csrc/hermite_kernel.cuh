@@ -154,6 +154,40 @@ __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const dou
     }
 }
 
+// Smallest squared pair separation of the system (bit pattern), positions only: the close-approach monitor of the
+// CARRY variant, whose evaluations are never taken at the post-step state.  Same pair schedule as eval_acc_jerk; no
+// return traffic (each lane keeps the minimum over the pairs it sees, monitor_flags reduces the flag over the lanes).
+template <int N, int L, int B>
+__device__ __forceinline__ u64 pair_r2min(const double (&x)[B][3], int l, int base, unsigned amask) {
+    constexpr bool PADDED = (L * B != N);
+    u64 r2min = ~0ull;
+    auto d2 = [](const double (&p)[3], const double (&q)[3]) {
+        const double dx = q[0] - p[0], dy = q[1] - p[1], dz = q[2] - p[2];
+        return fma(dz, dz, fma(dy, dy, dx * dx));
+    };
+#pragma unroll
+    for (int b = 0; b < B; ++b)
+#pragma unroll
+        for (int c = b + 1; c < B; ++c) min_bits(r2min, d2(x[b], x[c]), !PADDED || (l * B + c < N));
+    if constexpr (L > 1) {
+#pragma unroll
+        for (int s = 1; s <= (L - 1) / 2; ++s) {
+            int ls = l + s;
+            if (ls >= L) ls -= L;
+#pragma unroll
+            for (int c = 0; c < B; ++c) {
+                double xv[3];
+#pragma unroll
+                for (int q = 0; q < 3; ++q) xv[q] = __shfl_sync(amask, x[c][q], base + ls);
+                const bool vvalid = !PADDED || (ls * B + c < N);
+#pragma unroll
+                for (int b = 0; b < B; ++b) min_bits(r2min, d2(x[b], xv), vvalid && (!PADDED || (l * B + b < N)));
+            }
+        }
+    }
+    return r2min;
+}
+
 // Adaptive time step, Eq. 5: dt = tau [ sum_i |j_i|^2 / |a_i|^2 ]^(-1/2) over ALL bodies of the system
 // (R-A1), from the acceleration and jerk at the beginning of the step; bodies that feel no acceleration are left out
 // (R-A2).  Every lane of the system gathers the per-lane partial sums in the same (lane) order, so all of them take
@@ -216,8 +250,12 @@ __device__ __forceinline__ int monitor_flags(const double (&x)[B][3], u64 r2min,
 // instruction cache and the live register set at x, v, C_x, C_v, a, j).
 // ADAPT = true: the adaptive-step integrator (Eq. 5): p.dt is the step size scale tau, the step h and the ten
 // coefficients are per system and per step (registers) instead of launch constants.
-template <int N, int L, int B, bool UNROLL, int MAXT, int MINB, bool ADAPT = false>
+// CARRY = true: Alg. 2 exactly as printed (reading R6-alt): two evaluations per step; (a0, j0) of a step
+// are the (a2, j2) the previous step's last evaluation left in the registers; only the first step of a launch
+// evaluates at the state itself.  A third less pair work per step; the step is no longer a pure function of (x, v).
+template <int N, int L, int B, bool UNROLL, int MAXT, int MINB, bool ADAPT = false, bool CARRY = false>
 __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p) {
+    static_assert(!(ADAPT && CARRY), "the carried (a, j) are not kept across refills");
     constexpr int S = 32 / L;  // systems per warp
     constexpr bool PADDED = (L * B != N);
     const int lane = threadIdx.x & 31;
@@ -389,6 +427,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
             }
     };
 
+    bool fresh = true;  // CARRY: a, j do not yet belong to the current state (warp-uniform: start of the launch)
     if constexpr (UNROLL) {
         while (true) {
             if constexpr (ADAPT) {
@@ -400,7 +439,10 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 break;
             }
             if (active) {
-                eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
+                if (!CARRY || fresh)
+                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
+                else
+                    r2min = p.rc2_bits ? pair_r2min<N, L, B>(X, l, base, amask) : ~0ull;
                 accept_and_predict(amask);
                 if (active) {
                     eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
@@ -411,6 +453,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                     ++k;
                 }
             }
+            fresh = false;
         }
     } else {
         int phase = 0;  // warp-uniform: 0 = accept + predict, 1 and 2 = corrector iterations
@@ -427,7 +470,10 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 break;
             }
             if (active) {
-                eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
+                if (!CARRY || fresh || phase != 0)
+                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
+                else
+                    r2min = p.rc2_bits ? pair_r2min<N, L, B>(X, l, base, amask) : ~0ull;
                 if (phase == 0) {
                     accept_and_predict(amask);
                 } else {
@@ -439,6 +485,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 }
             }
             phase = phase == 2 ? 0 : phase + 1;
+            fresh = false;
         }
     }
     store_system();
