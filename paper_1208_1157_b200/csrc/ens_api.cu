@@ -331,7 +331,7 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
     a.order = nullptr;
     if (integrator == ENS_HERMITE_ADAPTIVE) {
         CU(cudaMemsetAsync(e->counter, 0, sizeof(unsigned long long), s));
-        if (!getenv("ENS_ADAPTIVE_UNORDERED")) {  // (the switch exists for the measurement in DESIGN.md §8)
+        if (!getenv("ENS_ADAPTIVE_UNORDERED") && e->v.n_sys <= 0x7fffffff) {  // int32 indices in the sort  // (the switch exists for the measurement in DESIGN.md §8)
             CU(ensd::adaptive_order(e->v, t_end, e->order, s));
             a.order = e->order.idx_out;
             e->launches += 1;  // the key kernel (the sort is cub's)

@@ -325,3 +325,18 @@ def test_streams_are_honoured():
         assert e.last_kernel_ms() > 0
     o = oracle.integrate(oracle.HERMITE, pos, vel, mass, dt=0.01, max_steps=300)
     assert rel_diff(d["pos"].cpu().numpy(), o["pos"]).max() <= 1e-11
+
+
+def test_two_million_systems_sampled_parity():
+    """A large ensemble (2^21 + 5 systems x 3 bodies, 940 MB of state incl. staging): indexing beyond 2^31 bytes per
+    array, ragged tail; sampled systems against the oracle, and the three step-loop kernels on the same ensemble."""
+    n_sys = (1 << 21) + 5
+    pos, vel, mass = W.generate(1, n_sys=n_sys)
+    idx = np.concatenate([np.arange(0, n_sys, 65536 + 1), [n_sys - 1, n_sys - 2]])
+    for integ, ointeg, dt in ((ens.HERMITE, oracle.HERMITE, 0.01), (ens.HERMITE_CARRY, oracle.HERMITE_CARRY, 0.01),
+                              (ens.HERMITE_ADAPTIVE, oracle.HERMITE_ADAPTIVE, 0.02)):
+        g = ens.run(integ, pos, vel, mass, dt=dt, steps=60, r_close=0.01, r_eject=100.0)
+        o = oracle.integrate(ointeg, pos[idx], vel[idx], mass[idx], dt=dt, max_steps=60, r_close=0.01, r_eject=100.0)
+        assert (g["status"] == ens.DONE_STEPS).all() and (g["nsteps"] == 60).all()
+        assert rel_diff(g["pos"][idx], o["pos"]).max() <= 1e-12 and rel_diff(g["vel"][idx], o["vel"]).max() <= 1e-12
+        assert np.abs(g["time"][idx] / o["time"] - 1).max() <= 1e-13
