@@ -25,7 +25,7 @@ _lock = threading.Lock()
 _lib = None
 
 ACTIVE, DONE_TIME, DONE_STEPS, STOP_CLOSE, STOP_EJECT, STOP_NONFINITE = range(6)
-HERMITE, MVS, HERMITE_ADAPTIVE, HERMITE_CARRY = 0, 1, 2, 3
+HERMITE, MVS, HERMITE_ADAPTIVE, HERMITE_CARRY, RKCK = 0, 1, 2, 3, 4
 # HERMITE_ADAPTIVE: `dt` is the step size scale tau of Eq. 5.  HERMITE_CARRY: Alg. 2 as printed, 2 evaluations per step.
 DOUBLE, LONG_DOUBLE = 0, 1
 
@@ -54,6 +54,8 @@ def _load():
         lib.orc_hermite_step.argtypes = [ci, d, d, d, cd, ci, ci]
         lib.orc_integrate.argtypes = [ci, cl, ci, d, d, d, d, i32, i64, cd, cd, cl, cd, cd, ci, ci]
         lib.orc_adaptive_dt.argtypes = [ci, d, d, d, cd, d, ci]
+        lib.orc_rkck_step.argtypes = [ci, d, d, d, cd, d, d, ci]
+        lib.orc_rkck_tableau.argtypes = [d, d, d, d]
         lib.orc_energy.argtypes = [cl, ci, d, d, d, d, d, ci]
         lib.orc_stumpff.argtypes = [cd, d, ci]
         lib.orc_kepler_drift.argtypes = [d, d, cd, cd, ci, ctypes.POINTER(ci)]
@@ -93,6 +95,22 @@ def hermite_step(x, v, m, h, n_corr=2, prec=DOUBLE):
     rc = _load().orc_hermite_step(m.shape[0], _p(x), _p(v), _p(m), float(h), int(n_corr), prec)
     assert rc == 0
     return x, v
+
+
+def rkck_step(x, v, m, h, prec=DOUBLE):
+    """One Cash-Karp step of one system; returns (x, v, errx, errv), err = 5th - 4th order solution."""
+    x, v, m = _f64(x).copy(), _f64(v).copy(), _f64(m)
+    ex, ev = np.empty_like(x), np.empty_like(v)
+    rc = _load().orc_rkck_step(m.shape[0], _p(x), _p(v), _p(m), float(h), _p(ex), _p(ev), prec)
+    assert rc == 0
+    return x, v, ex, ev
+
+
+def rkck_tableau():
+    """(c[6], a[6][5], b5[6], b4[6]) exactly as the oracle holds them."""
+    c, a, b5, b4 = np.empty(6), np.empty((6, 5)), np.empty(6), np.empty(6)
+    assert _load().orc_rkck_tableau(_p(c), _p(a), _p(b5), _p(b4)) == 0
+    return c, a, b5, b4
 
 
 def adaptive_dt(x, v, m, tau, prec=DOUBLE):

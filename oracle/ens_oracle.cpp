@@ -144,6 +144,89 @@ void hermite_step_carry(int n, R* x, R* v, const R* m, R h, R* a0, R* j0) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Fixed-step Runge-Kutta Cash-Karp (section 2.2.2, section 4.3.2): the explicit six-stage
+// embedded 4(5) pair of Cash & Karp (1990) applied to y = (x, v), y' = (v, a(x)); accelerations only, "six sub-steps
+// and six force evaluations for each step".  The step propagates the FIFTH-order solution, as the GSL rkck
+// stepper the paper says it follows does (reading R-RK1); the embedded fourth-order solution only serves the error
+// estimate err = y5 - y4 (returned for the tests; the adaptive controller is not defined by the paper: out of
+// scope).
+// ---------------------------------------------------------------------------------------------------
+template <class R>
+struct CashKarp {
+    R c[6], a[6][5], b5[6], b4[6];
+    CashKarp() {
+        const R z = 0;
+        const R cc[6] = {z, R(1) / 5, R(3) / 10, R(3) / 5, R(1), R(7) / 8};
+        const R aa[6][5] = {{z, z, z, z, z},
+                            {R(1) / 5, z, z, z, z},
+                            {R(3) / 40, R(9) / 40, z, z, z},
+                            {R(3) / 10, R(-9) / 10, R(6) / 5, z, z},
+                            {R(-11) / 54, R(5) / 2, R(-70) / 27, R(35) / 27, z},
+                            {R(1631) / 55296, R(175) / 512, R(575) / 13824, R(44275) / 110592, R(253) / 4096}};
+        const R bb5[6] = {R(37) / 378, z, R(250) / 621, R(125) / 594, z, R(512) / 1771};
+        const R bb4[6] = {R(2825) / 27648, z, R(18575) / 48384, R(13525) / 55296, R(277) / 14336, R(1) / 4};
+        for (int i = 0; i < 6; ++i) {
+            c[i] = cc[i];
+            b5[i] = bb5[i];
+            b4[i] = bb4[i];
+            for (int k = 0; k < 5; ++k) a[i][k] = aa[i][k];
+        }
+    }
+};
+
+template <class R>
+void eval_acc(int n, const R* x, const R* m, R* a) {  // Eq. 1 (R1), planets ascending then the star
+    for (int i = 0; i < n; ++i) {
+        R ai[3] = {0, 0, 0};
+        for (int kk = 1; kk <= n; ++kk) {
+            const int k = (kk == n) ? 0 : kk;
+            if (k == i) continue;
+            R dx[3];
+            for (int c = 0; c < 3; ++c) dx[c] = x[3 * k + c] - x[3 * i + c];
+            const R r2 = dx[0] * dx[0] + dx[1] * dx[1] + dx[2] * dx[2];
+            const R rinv = rsqrt_exact(r2);
+            const R rinv3 = rinv * rinv * rinv;
+            for (int c = 0; c < 3; ++c) ai[c] += m[k] * rinv3 * dx[c];
+        }
+        for (int c = 0; c < 3; ++c) a[3 * i + c] = ai[c];
+    }
+}
+
+// one step; errx / errv (may be null) receive y5 - y4
+template <class R>
+void rkck_step(int n, R* x, R* v, const R* m, R h, R* errx = nullptr, R* errv = nullptr) {
+    static const CashKarp<R> T;
+    const int d = 3 * n;
+    std::vector<R> kx(6 * d), kv(6 * d), xs(d), vs(d);
+    for (int i = 0; i < 6; ++i) {
+        for (int q = 0; q < d; ++q) {
+            R sx = 0, sv = 0;
+            for (int k = 0; k < i; ++k) {
+                sx += T.a[i][k] * kx[k * d + q];
+                sv += T.a[i][k] * kv[k * d + q];
+            }
+            xs[q] = x[q] + h * sx;
+            vs[q] = v[q] + h * sv;
+        }
+        for (int q = 0; q < d; ++q) kx[i * d + q] = vs[q];      // x' = v
+        eval_acc(n, xs.data(), m, kv.data() + i * d);           // v' = a(x)
+    }
+    for (int q = 0; q < d; ++q) {
+        R x5 = 0, v5 = 0, x4 = 0, v4 = 0;
+        for (int i = 0; i < 6; ++i) {
+            x5 += T.b5[i] * kx[i * d + q];
+            v5 += T.b5[i] * kv[i * d + q];
+            x4 += T.b4[i] * kx[i * d + q];
+            v4 += T.b4[i] * kv[i * d + q];
+        }
+        if (errx) errx[q] = h * (x5 - x4);
+        if (errv) errv[q] = h * (v5 - v4);
+        x[q] += h * x5;
+        v[q] += h * v5;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Adaptive time step, Eq. 5:  dt = tau [ sum_i |j_i0|^2 / |a_i0|^2 ]^(-1/2),  i over ALL bodies of the
 // system ("i indexes a body in the system", the star included: reading R-A1), a_i0 and j_i0 evaluated at the
 // beginning of the step ("uses only the values at the beginning of the time step").  tau carries the
@@ -436,6 +519,9 @@ void run_system(int integrator, int n, double* pos, double* vel, const double* m
         if (integrator == 0) {
             hermite_step(n, x.data(), v.data(), m.data(), h, n_corr);
             xmon = x.data();
+        } else if (integrator == 4) {  // fixed-step Runge-Kutta Cash-Karp
+            rkck_step(n, x.data(), v.data(), m.data(), h);
+            xmon = x.data();
         } else if (integrator == 3) {  // Alg. 2 as printed: 2 evaluations per step, (a, j) carried
             hermite_step_carry(n, x.data(), v.data(), m.data(), h, ca.data(), cj.data());
             xmon = x.data();
@@ -493,12 +579,13 @@ int orc_hermite_step(int n, double* x, double* v, const double* m, double h, int
 }
 
 // integrator: 0 = Hermite (fixed step dt), 1 = MVS, 2 = adaptive Hermite (dt = tau of Eq. 5),
-// 3 = Hermite with 2 evaluations per step (Alg. 2 as printed; a, j carried from step to step).  status/nsteps/time are in-out ([n_sys]); status STOP_* is sticky.
+// 3 = Hermite with 2 evaluations per step (Alg. 2 as printed; a, j carried from step to step),
+// 4 = fixed-step Runge-Kutta Cash-Karp (fifth-order solution propagated).  status/nsteps/time are in-out ([n_sys]); status STOP_* is sticky.
 int orc_integrate(int integrator, int64_t n_sys, int n, double* pos, double* vel, const double* mass, double* time,
                   int32_t* status, int64_t* nsteps, double dt, double t_end, int64_t max_steps, double r_close,
                   double r_eject, int prec, int nthreads) {
     if (n_sys < 0 || n < 2 || !pos || !vel || !mass || !time || !status || !nsteps) return -1;
-    if (!(dt != 0) || !std::isfinite(dt) || max_steps < 0 || (integrator < 0 || integrator > 3)) return -1;
+    if (!(dt != 0) || !std::isfinite(dt) || max_steps < 0 || (integrator < 0 || integrator > 4)) return -1;
     if (nthreads < 1) nthreads = 1;
 #pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads)
     for (int64_t s = 0; s < n_sys; ++s) {
@@ -509,6 +596,30 @@ int orc_integrate(int integrator, int64_t n_sys, int n, double* pos, double* vel
             run_system<double>(integrator, n, p, w, mm, time + s, status + s, nsteps + s, dt, t_end, max_steps, r_close, r_eject, 2);
         else
             run_system<long double>(integrator, n, p, w, mm, time + s, status + s, nsteps + s, dt, t_end, max_steps, r_close, r_eject, 2);
+    }
+    return 0;
+}
+
+// one Cash-Karp step of one system (test hook); errx, errv receive the embedded error estimate y5 - y4
+int orc_rkck_step(int n, double* x, double* v, const double* m, double h, double* errx, double* errv, int prec) {
+    if (n < 2 || !x || !v || !m || !errx || !errv) return -1;
+    if (prec == 0) {
+        rkck_step<double>(n, x, v, m, h, errx, errv);
+    } else {
+        std::vector<long double> X(x, x + 3 * n), V(v, v + 3 * n), M(m, m + n), EX(3 * n), EV(3 * n);
+        rkck_step<long double>(n, X.data(), V.data(), M.data(), (long double)h, EX.data(), EV.data());
+        for (int q = 0; q < 3 * n; ++q) { x[q] = (double)X[q]; v[q] = (double)V[q]; errx[q] = (double)EX[q]; errv[q] = (double)EV[q]; }
+    }
+    return 0;
+}
+
+// the Cash-Karp tableau as the oracle holds it (test hook): c[6], a[6][5] row-major, b5[6], b4[6]
+int orc_rkck_tableau(double* c, double* a, double* b5, double* b4) {
+    if (!c || !a || !b5 || !b4) return -1;
+    const CashKarp<long double> T;
+    for (int i = 0; i < 6; ++i) {
+        c[i] = (double)T.c[i]; b5[i] = (double)T.b5[i]; b4[i] = (double)T.b4[i];
+        for (int k = 0; k < 5; ++k) a[5 * i + k] = (double)T.a[i][k];
     }
     return 0;
 }
