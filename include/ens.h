@@ -38,7 +38,7 @@ extern "C" {
 typedef struct ens ens_t; /* opaque */
 
 enum { ENS_OK = 0, ENS_EINVAL = -1, ENS_ENOMEM = -2, ENS_ECUDA = -3, ENS_ESTATE = -4, ENS_EUNSUPPORTED = -5 };
-enum { ENS_HERMITE = 0, ENS_MVS = 1, ENS_HERMITE_ADAPTIVE = 2, ENS_HERMITE_CARRY = 3 };
+enum { ENS_HERMITE = 0, ENS_MVS = 1, ENS_HERMITE_ADAPTIVE = 2, ENS_HERMITE_CARRY = 3, ENS_RKCK = 4 };
 enum { ENS_HOST = 0, ENS_DEVICE = 1 };
 /* per-system status (Alg. 1 "state").  DONE_* become ACTIVE again at the next ens_integrate;
  * STOP_* are sticky until ens_set_state. */
@@ -85,7 +85,8 @@ ENS_API int ens_set_monitors(ens_t *e, double r_close, double r_eject);
  * takes its own steps, and `time` advances by the step actually taken; ENS_HERMITE_CARRY = Alg. 2 exactly as printed
  * (reading R6-alt): fixed step, TWO evaluations per step, a^(0), j^(0) of a step being the a^(2), j^(2)
  * the previous step left behind (only the first step of a call evaluates at the state itself, so a run split over
- * two calls is not bit-identical to the unsplit one).
+ * two calls is not bit-identical to the unsplit one); ENS_RKCK = fixed-step Runge-Kutta Cash-Karp (P:L93-97,
+ * P:L246-248): six acceleration evaluations per step, no jerk, the fifth-order solution propagated (R-RK1).
  * EINVAL: NULL handle, unknown integrator, dt == 0 or non-finite, NaN t_end, max_steps < 0.
  * ESTATE: no state was set.  ECUDA: launch failed. */
 ENS_API int ens_integrate(ens_t *e, int integrator, double dt, double t_end, int64_t max_steps, void *stream);

@@ -165,7 +165,7 @@ struct ens {
     // device staging (AoS) for host-space calls, allocated on first use
     double* stage;        // [n_sys * n_body * 7] : pos | vel | mass
     double* stage_small;  // [n_sys * 4] : time / E | L   (also int32 status, int64 nsteps reuse)
-    ensd::KernelInfo hermite, hermite_adaptive, hermite_carry, mvs;
+    ensd::KernelInfo hermite, hermite_adaptive, hermite_carry, rkck, mvs;
     unsigned long long* counter;  // work counter of the adaptive kernels
     ensd::OrderBuffers order;     // hand-out order of the adaptive kernels (allocated on first use)
     int threads_override;
@@ -242,6 +242,7 @@ int ens_create(int64_t n_sys, int n_body, ens_t** out) {
     e->hermite = ensd::hermite_kernel_for(n_body, 0);
     e->hermite_adaptive = ensd::hermite_kernel_for(n_body, 1);
     e->hermite_carry = ensd::hermite_kernel_for(n_body, 2);
+    e->rkck = ensd::rkck_kernel_for(n_body);
     e->mvs = ensd::mvs_kernel_for(n_body);
     const char* env = getenv("ENS_THREADS");
     e->threads_override = env ? atoi(env) : 0;
@@ -313,7 +314,7 @@ int ens_set_state(ens_t* e, const double* pos, const double* vel, const double* 
 }
 
 int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max_steps, void* stream) {
-    if (!e || integrator < ENS_HERMITE || integrator > ENS_HERMITE_CARRY) return ENS_EINVAL;
+    if (!e || integrator < ENS_HERMITE || integrator > ENS_RKCK) return ENS_EINVAL;
     if (!(dt != 0.0) || !std::isfinite(dt) || std::isnan(t_end) || max_steps < 0) return ENS_EINVAL;
     if (!e->have_state) return ENS_ESTATE;
     cudaStream_t s = (cudaStream_t)stream;
@@ -340,12 +341,15 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
     const ensd::KernelInfo& ki = integrator == ENS_HERMITE            ? e->hermite
                                  : integrator == ENS_HERMITE_ADAPTIVE ? e->hermite_adaptive
                                  : integrator == ENS_HERMITE_CARRY    ? e->hermite_carry
+                                 : integrator == ENS_RKCK             ? e->rkck
                                                                       : e->mvs;
     if (!ki.fn) return ENS_EUNSUPPORTED;
     const int threads = e->threads_override ? e->threads_override : ki.threads;
     CU(cudaEventRecord(e->ev0, s));
     cudaError_t err = integrator == ENS_MVS
                           ? ensd::launch_mvs(e->v, a, threads, s, &e->last_blocks)
+                      : integrator == ENS_RKCK
+                          ? ensd::launch_rkck(e->v, a, threads, s, &e->last_blocks)
                           : ensd::launch_hermite(e->v, a, integrator == ENS_HERMITE_ADAPTIVE ? 1 : integrator == ENS_HERMITE_CARRY ? 2 : 0,
                                                  threads, s, &e->last_blocks);
     if (err != cudaSuccess) return cuda_fail(err, "ens_integrate launch");
@@ -419,6 +423,7 @@ int ens_get_info(const ens_t* e, int64_t out[8]) {
     const ensd::KernelInfo& ki = (e->last_fn && e->last_fn == e->mvs.fn)                ? e->mvs
                                  : (e->last_fn && e->last_fn == e->hermite_adaptive.fn) ? e->hermite_adaptive
                                  : (e->last_fn && e->last_fn == e->hermite_carry.fn)    ? e->hermite_carry
+                                 : (e->last_fn && e->last_fn == e->rkck.fn)             ? e->rkck
                                                                                         : e->hermite;
     const int threads = e->threads_override ? e->threads_override : ki.threads;
     out[0] = e->v.n_pad;

@@ -80,6 +80,8 @@ void adaptive_order_free(OrderBuffers& ob);
 KernelInfo hermite_kernel_for(int n_body, int mode);  // mode: 0 fixed step, 1 adaptive, 2 carried a/j
 cudaError_t launch_hermite(const View& v, const StepArgs& a, int mode, int threads, cudaStream_t s,
                            int64_t* blocks_out);
+KernelInfo rkck_kernel_for(int n_body);
+cudaError_t launch_rkck(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out);
 KernelInfo mvs_kernel_for(int n_body);
 cudaError_t launch_mvs(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out);
 

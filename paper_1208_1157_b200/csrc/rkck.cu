@@ -1,0 +1,129 @@
+// rkck.cu — instantiations of the fused Cash-Karp step-loop kernel, the n_body -> (L, B) dispatch and the tableau.
+#include "rkck_kernel.cuh"
+
+namespace ensd {
+
+namespace {
+
+// n_body -> lanes per system L (odd), bodies per lane B, L * B >= n_body.  Five stage accelerations per body live in
+// registers, so a lane holds fewer bodies than in the Hermite kernel.
+template <int N> struct RkShape;
+#define ENS_RK_SHAPE(N_, L_, B_, THREADS_, MAXREG_)                                \
+    template <> struct RkShape<N_> {                                               \
+        static constexpr int L = L_, B = B_, THREADS = THREADS_, MAXREG = MAXREG_; \
+    };
+#ifndef ENS_RK3_THREADS
+#define ENS_RK3_THREADS 64
+#endif
+#ifndef ENS_RK3_MAXREG
+#define ENS_RK3_MAXREG 255
+#endif
+//           N   L  B  threads maxRegisters
+ENS_RK_SHAPE(2, 1, 2, 64, 255)
+ENS_RK_SHAPE(3, 1, 3, ENS_RK3_THREADS, ENS_RK3_MAXREG)
+ENS_RK_SHAPE(4, 1, 4, 64, 255)
+ENS_RK_SHAPE(5, 3, 2, 64, 255)
+ENS_RK_SHAPE(6, 3, 2, 64, 255)
+ENS_RK_SHAPE(7, 3, 3, 64, 255)
+ENS_RK_SHAPE(8, 3, 3, 64, 255)
+ENS_RK_SHAPE(9, 3, 3, 64, 255)
+ENS_RK_SHAPE(10, 5, 2, 64, 255)
+ENS_RK_SHAPE(11, 5, 3, 64, 255)
+ENS_RK_SHAPE(12, 5, 3, 64, 255)
+ENS_RK_SHAPE(13, 5, 3, 64, 255)
+ENS_RK_SHAPE(14, 5, 3, 64, 255)
+ENS_RK_SHAPE(15, 5, 3, 64, 255)
+ENS_RK_SHAPE(16, 5, 4, 64, 255)
+#undef ENS_RK_SHAPE
+
+template <int N>
+constexpr auto kernel_ptr() {
+    using S = RkShape<N>;
+    return &rkck_kernel<N, S::L, S::B, S::MAXREG>;
+}
+
+template <int N>
+KernelInfo info_of() {
+    using S = RkShape<N>;
+    KernelInfo k;
+    k.fn = (const void*)kernel_ptr<N>();
+    k.shape.L = S::L;
+    k.shape.B = S::B;
+    k.threads = S::THREADS;
+    return k;
+}
+
+// Cash & Karp's tableau (the published rationals) and the products the kernel uses, all formed in long double and
+// rounded once.
+RkCoef coefficients(double h) {
+    typedef long double R;
+    const R A[6][5] = {{0, 0, 0, 0, 0},
+                       {R(1) / 5, 0, 0, 0, 0},
+                       {R(3) / 40, R(9) / 40, 0, 0, 0},
+                       {R(3) / 10, R(-9) / 10, R(6) / 5, 0, 0},
+                       {R(-11) / 54, R(5) / 2, R(-70) / 27, R(35) / 27, 0},
+                       {R(1631) / 55296, R(175) / 512, R(575) / 13824, R(44275) / 110592, R(253) / 4096}};
+    const R b[6] = {R(37) / 378, 0, R(250) / 621, R(125) / 594, 0, R(512) / 1771};
+    RkCoef q;
+    const R H = h, H2 = H * H;
+    for (int i = 0; i < 6; ++i) {
+        R c = 0;
+        for (int j = 0; j < i; ++j) c += A[i][j];
+        q.ch[i] = (double)(c * H);
+        q.hb[i] = (double)(b[i] * H);
+        for (int ll = 0; ll < 4; ++ll) {
+            R s = 0;
+            for (int j = ll + 1; j < i; ++j) s += A[i][j] * A[j][ll];
+            q.h2AA[i][ll] = (double)(s * H2);
+        }
+    }
+    for (int ll = 0; ll < 5; ++ll) {
+        R s = 0;
+        for (int i = ll + 1; i < 6; ++i) s += b[i] * A[i][ll];
+        q.h2bA[ll] = (double)(s * H2);
+    }
+    return q;
+}
+
+template <int N>
+cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
+    using S = RkShape<N>;
+    if (threads > S::THREADS) threads = S::THREADS;  // blocks must not exceed 65536 / MAXREG threads
+    const int64_t sys_per_warp = 32 / S::L;
+    const int64_t warps = (v.n_sys + sys_per_warp - 1) / sys_per_warp;
+    const int wpb = threads / 32;
+    const int64_t blocks = (warps + wpb - 1) / wpb;
+    if (blocks_out) *blocks_out = blocks;
+    kernel_ptr<N>()<<<(unsigned)blocks, threads, 0, s>>>(v, a, coefficients(a.dt));
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+#define ENS_FOR_EACH_N(X) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
+
+KernelInfo rkck_kernel_for(int n_body) {
+    switch (n_body) {
+#define X(N_) \
+    case N_: return info_of<N_>();
+        ENS_FOR_EACH_N(X)
+#undef X
+    }
+    KernelInfo none;
+    none.fn = nullptr;
+    none.shape.L = none.shape.B = 0;
+    none.threads = 0;
+    return none;
+}
+
+cudaError_t launch_rkck(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
+    switch (v.n_body) {
+#define X(N_) \
+    case N_: return launch_n<N_>(v, a, threads, s, blocks_out);
+        ENS_FOR_EACH_N(X)
+#undef X
+    }
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace ensd

@@ -13,7 +13,7 @@ import numpy as np
 import torch
 
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, EUNSUPPORTED = 0, -1, -2, -3, -4, -5
-HERMITE, MVS, HERMITE_ADAPTIVE, HERMITE_CARRY = 0, 1, 2, 3  # HERMITE_ADAPTIVE: `dt` is the step size scale tau of Eq. 5
+HERMITE, MVS, HERMITE_ADAPTIVE, HERMITE_CARRY, RKCK = 0, 1, 2, 3, 4  # HERMITE_ADAPTIVE: `dt` is the step size scale tau of Eq. 5
 HOST, DEVICE = 0, 1
 ACTIVE, DONE_TIME, DONE_STEPS, STOP_CLOSE, STOP_EJECT, STOP_NONFINITE = range(6)
 
