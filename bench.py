@@ -371,6 +371,18 @@ def main():
                 ea.close()
             except ens.EnsError as ex:
                 others["hermite_adaptive_131072x3"] = {"unavailable": str(ex)}
+            # the 2-evaluation Hermite and the Cash-Karp kernels on the metric's own ensemble (kernel time, full 10^4 steps)
+            for integ, key in ((ens.HERMITE_CARRY, "hermite_carry_131072x3"), (ens.RKCK, "rkck_131072x3")):
+                try:
+                    msk = []
+                    for _ in range(2):
+                        e.set_state(d_pos, d_vel, d_mass, stream=stream)
+                        e.integrate(integ, c.dt, c.steps, stream=stream)
+                        msk.append(e.last_kernel_ms())
+                    others[key] = {"value": n_sys * c.steps / (msk[-1] * 1e-3), "unit": "system-steps/s",
+                                   "kernel_ms": msk[-1], "regs": e.info()["regs"]}
+                except ens.EnsError as ex:
+                    others[key] = {"unavailable": str(ex)}
             line["other_workloads"] = others
             if W.CONFIGS[4].name in others:
                 line["mvs"] = dict(others[W.CONFIGS[4].name], workload=W.CONFIGS[4].name)

@@ -16,7 +16,7 @@ template <int N> struct RkShape;
 #define ENS_RK3_THREADS 64
 #endif
 #ifndef ENS_RK3_MAXREG
-#define ENS_RK3_MAXREG 255
+#define ENS_RK3_MAXREG 168
 #endif
 //           N   L  B  threads maxRegisters
 ENS_RK_SHAPE(2, 1, 2, 64, 255)
