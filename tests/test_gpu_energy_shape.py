@@ -1,0 +1,58 @@
+"""Paper Table 1 / Fig. 2, shape only: over a long run of the section-5.1 systems the MVS energy error stays
+roughly constant while the adaptive Hermite error accumulates slowly.  Run on the GPU in segments through the
+C ABI (repeated ens_integrate + ens_energy calls: the 'log' role of the paper's monitors, is played by the
+ensemble itself: DESIGN.md section 3, R-L1).  The printed magnitudes are parity-unpinned (tests/golden/table1_energy.txt)."""
+import numpy as np
+import pytest
+
+from paper_1208_1157_b200 import ens
+from paper_1208_1157_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _phased_paper_systems(n_sys, seed):
+    """Section 5.1 initial conditions with seeded orbital phases (the paper gives none)."""
+    rng = np.random.default_rng(seed)
+    pos, vel, mass = W.paper_ics(3, n_sys=n_sys)
+    for b in (1, 2):
+        ph = rng.uniform(0, 2 * np.pi, n_sys)
+        c, s = np.cos(ph), np.sin(ph)
+        for arr in (pos, vel):
+            x, y = arr[:, b, 0].copy(), arr[:, b, 1].copy()
+            arr[:, b, 0], arr[:, b, 1] = c * x - s * y, s * x + c * y
+    return pos, vel, mass
+
+
+def _segments(integrator, dt, n_seg, steps=None, seg_t=None):
+    pos, vel, mass = _phased_paper_systems(128, 1)
+    out = []
+    with ens.Ensemble(128, 3) as e:
+        e.set_state(pos, vel, mass)
+        E0, L0 = e.energy()
+        for seg in range(n_seg):
+            if seg_t is None:
+                e.integrate(integrator, dt, steps)
+            else:
+                e.integrate(integrator, dt, 10**9, t_end=(seg + 1) * seg_t)
+            E, L = e.energy()
+            out.append((np.abs((E - E0) / E0), np.abs(L - L0).max(axis=1) / np.abs(L0).max(axis=1)))
+        st = e.get_state()
+    return out, st
+
+
+def test_mvs_energy_error_is_bounded_and_flat():
+    out, st = _segments(ens.MVS, 0.01, 10, steps=40000)  # the paper's MVS step, t = 4000 = 640 inner orbits
+    med = np.array([np.median(dE) for dE, _ in out])
+    assert (st["status"] == ens.DONE_STEPS).all() and (st["nsteps"] == 400000).all()
+    assert med.max() / med.min() < 3.0 and med[5:].mean() / med[:5].mean() < 1.5, med   # "roughly constant"
+    assert max(dE.max() for dE, _ in out) < 2e-7                                          # ~ m (n dt)^2, bounded
+    assert max(dL.max() for _, dL in out) < 5e-10   # accumulated rounding only (the oracle reaches 4e-11 on this run)
+
+
+def test_adaptive_hermite_energy_error_accumulates_slowly():
+    out, st = _segments(ens.HERMITE_ADAPTIVE, 0.017, 10, seg_t=400.0)  # the paper's tau
+    med = np.array([np.median(dE) for dE, _ in out])
+    assert (st["status"] == ens.DONE_TIME).all()
+    assert med[-1] / med[0] > 3.0 and (np.diff(med) > -0.3 * med[:-1]).all(), med  # "slow accumulation"
+    assert med[-1] < 1e-9
