@@ -8,15 +8,22 @@ typedef unsigned long long u64;
 
 __device__ __forceinline__ u64 dbits(double x) { return (u64)__double_as_longlong(x); }
 
-// FP64 reciprocal square root (P:L276 used the Fermi hardware rsqrt; R14): MUFU.RSQ seed of the value rounded
-// to FP32 (relative error <= 2^-22) and one cubic Newton-Halley step in FP64,
-//   e = 1 - r2 y0^2,  y = y0 + y0 e (1/2 + 3/8 e),   remaining error ~ (5/16) e^3 < 2^-66 plus rounding: <= 1 ulp
-// (tests/test_gpu_device_functions.py measures it).  Valid for r2 inside the FP32 normal range, 1.2e-38 < r2 <
-// 3.4e38, i.e. separations between 1e-19 and 1e19 length units.
+// FP64 reciprocal square root (P:L276 used the Fermi hardware rsqrt; R14): MUFU.RSQ64H seed (the approximation unit
+// reads the high word of the double: no F2F round trip, full FP64 exponent range, relative error ~2^-20) and one
+// cubic Newton-Halley step in FP64,
+//   e = 1 - r2 y0^2,  y = y0 + y0 e (1/2 + 3/8 e),   remaining error ~ (5/16) e^3 < 2^-61 plus rounding: <= 1 ulp
+// (tests/test_gpu_hermite.py::test_rsqrt_within_one_ulp measures it).  Valid for normal, finite r2 > 0.
+// -DENS_SEED_F32 selects the older seed (FP32 MUFU.RSQ of the value rounded to float: two extra F2F per call, and
+// r2 restricted to the FP32 range); it was 2-6 % slower in every kernel.
 __device__ __forceinline__ double rsqrt_f64(double r2) {
+    double y0;
+#ifndef ENS_SEED_F32
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(r2));
+#else
     float s;
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(__double2float_rn(r2)));
-    const double y0 = (double)s;
+    y0 = (double)s;
+#endif
     const double t = r2 * y0;
     const double e = fma(-t, y0, 1.0);
     const double p = fma(0.375, e, 0.5);
@@ -24,15 +31,20 @@ __device__ __forceinline__ double rsqrt_f64(double r2) {
     return fma(q, p, y0);
 }
 
-// FP64 reciprocal without the IEEE divide sequence: MUFU.RCP seed of the value rounded to FP32 (relative error
-// <= 2^-22), then y = y0 + y0 e (1 + e), e = 1 - x y0: remaining error e^3 < 2^-66 plus rounding (<= 1 ulp).
-// REFINE = false stops at y0 + y0 e (relative error 2^-44): enough for a Newton step, which is self-correcting.
-// Valid for |x| inside the FP32 normal range.
+// FP64 reciprocal without the IEEE divide sequence: MUFU.RCP64H seed (relative error ~2^-20), then
+// y = y0 + y0 e (1 + e), e = 1 - x y0: remaining error e^3 < 2^-60 plus rounding (<= 1 ulp).
+// REFINE = false stops at y0 + y0 e (relative error ~2^-40): enough for a Newton step, which is self-correcting.
+// Valid for normal, finite x != 0.
 template <bool REFINE>
 __device__ __forceinline__ double rcp_f64(double x) {
+#ifndef ENS_SEED_F32
+    double y0;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
+#else
     float s;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(__double2float_rn(x)));
     const double y0 = (double)s;
+#endif
     const double e = fma(-x, y0, 1.0);
     const double q = y0 * e;
     if constexpr (REFINE) return fma(q, 1.0 + e, y0);

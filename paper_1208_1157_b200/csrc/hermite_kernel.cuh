@@ -191,8 +191,7 @@ __device__ __forceinline__ u64 pair_r2min(const double (&x)[B][3], int l, int ba
 // Adaptive time step, Eq. 5: dt = tau [ sum_i |j_i|^2 / |a_i|^2 ]^(-1/2) over ALL bodies of the system
 // (R-A1), from the acceleration and jerk at the beginning of the step; bodies that feel no acceleration are left out
 // (R-A2).  Every lane of the system gathers the per-lane partial sums in the same (lane) order, so all of them take
-// bit-identical steps.  Reciprocal and reciprocal square root come from the FP32 seeds + FP64 refinement (<= 1 ulp)
-// inside the FP32 range, from the IEEE sequences outside it.
+// bit-identical steps.  Reciprocal and reciprocal square root are the seeded + refined ones of ens_device.cuh (<= 1 ulp).
 template <int N, int L, int B>
 __device__ __forceinline__ double adaptive_dt(const double (&a)[B][3], const double (&j)[B][3], double tau, int l,
                                               int base, unsigned amask) {
@@ -202,8 +201,7 @@ __device__ __forceinline__ double adaptive_dt(const double (&a)[B][3], const dou
     for (int b = 0; b < B; ++b) {
         const double a2 = fma(a[b][2], a[b][2], fma(a[b][1], a[b][1], a[b][0] * a[b][0]));
         const double j2 = fma(j[b][2], j[b][2], fma(j[b][1], j[b][1], j[b][0] * j[b][0]));
-        double ia2 = rcp_f64<true>(a2);
-        if (!(a2 > 1e-30 && a2 < 1e30)) ia2 = a2 > 0.0 ? 1.0 / a2 : 0.0;
+        const double ia2 = a2 > 1e-290 ? rcp_f64<true>(a2) : 0.0;  // R-A2: no acceleration, no term
         if (!PADDED || (l * B + b < N)) part = fma(j2, ia2, part);
     }
     double sum = part;
@@ -212,9 +210,7 @@ __device__ __forceinline__ double adaptive_dt(const double (&a)[B][3], const dou
 #pragma unroll
         for (int i = 1; i < L; ++i) sum += __shfl_sync(amask, part, base + i);
     }
-    double y = rsqrt_f64(sum);
-    if (!(sum > 1e-30 && sum < 1e30)) y = 1.0 / sqrt(sum);
-    return tau * y;
+    return tau * rsqrt_f64(sum);
 }
 
 // bits: 1 = close approach, 2 = ejection, 4 = non-finite position; OR-reduced over the lanes of the system.
