@@ -258,7 +258,9 @@ def main():
                        "steps_per_launch": c.steps, "monitors": {"r_close": c.r_close, "r_eject": c.r_eject},
                        "l2": "flushed between timed iterations (512 MB memset); state lives in registers",
                        "parallelism": f"independent ensembles x{world}" if world > 1 else "single GPU"},
-            "clocks": clocks, "gpu_launches": launches, "wall_s_timed_region": t_wall,
+            "clocks": clocks, "gpu_launches": launches,
+            # context only (other hardware, derived): never the target, never vs_baseline
+            "paper_context": {"m2070_system_steps_per_s_derived": 3.65e6, "source": "P:L347 Table 3 / P:L321"}, "wall_s_timed_region": t_wall,
             "pair_interactions_per_s": value * (n_body * (n_body - 1) // 2) * 3,
             "kernel": {"lanes_per_system": info["lanes_per_system"], "bodies_per_lane": info["bodies_per_lane"],
                        "threads": info["threads"], "blocks": info["blocks"], "regs": info["regs"],
@@ -274,7 +276,7 @@ def main():
             roof = {"bound": "alu", "kernel": f"hermite_kernel<{n_body},{info['lanes_per_system']},{info['bodies_per_lane']}>", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
                     "frac": ach_tf / peak_tf,
                     # ncu dram__bytes_read.sum + dram__bytes_write.sum of this kernel, one launch, config 1
-                    # (profiles/r1g_hermite_cfg1_ncu_full.txt); the store drains from L2 after the kernel ends
+                    # (profiles/r1i_hermite_cfg1_ncu_full.txt); the store drains from L2 after the kernel ends
                     "traffic": 24.7e6 if CFG == 1 else None,
                     "peak_source": f"derived: {props.multi_processor_count} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 flop x "
                                    f"{clocks.get('sm_max_mhz') or 1965.0:.0f} MHz (DESIGN.md §8)",
