@@ -57,7 +57,8 @@ __device__ __forceinline__ double pair_acc_jerk(const double (&xi)[3], const dou
 
 // Acceleration and jerk of the B bodies this lane owns, every pair of the system once.
 // l = lane index inside the system (0..L-1), base = first lane of the system in the warp, amask = active lanes.
-template <int N, int L, int B>
+// TRACK = false skips the minimum pair distance (only a step's first evaluation feeds the monitor).
+template <int N, int L, int B, bool TRACK = true>
 __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const double (&v)[B][3], const double (&m)[B],
                                               double (&a)[B][3], double (&j)[B][3], u64& r2min, int l, int base,
                                               unsigned amask) {
@@ -66,7 +67,7 @@ __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const dou
     for (int b = 0; b < B; ++b)
 #pragma unroll
         for (int c = 0; c < 3; ++c) a[b][c] = j[b][c] = 0.0;
-    r2min = ~0ull;
+    if constexpr (TRACK) r2min = ~0ull;
 
     // Cross-lane schedule (L > 1), written so that shuffle latency hides behind FP64 work of the same warp (a warp
     // issues in order: an instruction that waits on a shuffle blocks everything behind it):
@@ -99,7 +100,7 @@ __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const dou
 #pragma unroll
         for (int c = b + 1; c < B; ++c) {
             const double r2 = pair_acc_jerk(x[b], v[b], m[b], a[b], j[b], x[c], v[c], m[c], a[c], j[c]);
-            min_bits(r2min, r2, !PADDED || (l * B + c < N));
+            if constexpr (TRACK) min_bits(r2min, r2, !PADDED || (l * B + c < N));
         }
     }
 
@@ -124,7 +125,7 @@ __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const dou
                 for (int b = 0; b < B; ++b) {
                     const double r2 = pair_acc_jerk(x[b], v[b], m[b], a[b], j[b], xv[buf][c], vv[buf][c], mv[buf][c],
                                                     av[c], jv[c]);
-                    min_bits(r2min, r2, vvalid && (!PADDED || (l * B + b < N)));
+                    if constexpr (TRACK) min_bits(r2min, r2, vvalid && (!PADDED || (l * B + b < N)));
                 }
             }
             if (s > 1) {
@@ -441,9 +442,9 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                     r2min = p.rc2_bits ? pair_r2min<N, L, B>(X, l, base, amask) : ~0ull;
                 accept_and_predict(amask);
                 if (active) {
-                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
+                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, amask);
                     correct();
-                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
+                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, amask);
                     correct();
                     t += h;
                     ++k;
