@@ -96,6 +96,31 @@ ENS_API int ens_integrate(ens_t *e, int integrator, double dt, double t_end, int
 ENS_API int ens_get_state(const ens_t *e, double *pos, double *vel, double *time, int32_t *status, int64_t *nsteps,
                   int memspace, void *stream);
 
+/* ---- state log (the "log" action of the paper's monitors; readings R-L1, R-L2 of DESIGN.md) ---------- */
+enum { ENS_LOG_SNAPSHOTS = 1, /* every system that advanced, after every segment */
+       ENS_LOG_STOPS = 2      /* systems a stop monitor halted (status >= ENS_STOP_CLOSE), once, with their stop state */ };
+
+/* Allocate (capacity > 0) or free (capacity == 0) the device log buffer of `capacity` records and empty it.  A
+ * record is (system index, its total step count, its time, its status, pos [n_body][3], vel [n_body][3]).  Waits for
+ * `stream` first.  EINVAL: NULL handle or capacity < 0.  ENOMEM. */
+ENS_API int ens_log_enable(ens_t *e, int64_t capacity, void *stream);
+
+/* ens_integrate in segments of `log_every` steps; after each segment a kernel on the same stream appends one record
+ * for every system selected by `what` (ENS_LOG_* bits) that advanced since its last record.  Everything is enqueued:
+ * no host round trip between segments.  Records beyond the capacity are dropped and counted.  Results are
+ * bit-identical to one ens_integrate of max_steps for ENS_HERMITE, ENS_HERMITE_ADAPTIVE, ENS_RKCK and ENS_MVS up to
+ * its coordinate round trip (their step is a pure function of the state); ENS_HERMITE_CARRY re-evaluates at every
+ * segment start.  EINVAL: as ens_integrate, or log_every < 1, or no ENS_LOG_* bit.  ESTATE: no log buffer / state. */
+ENS_API int ens_integrate_logged(ens_t *e, int integrator, double dt, double t_end, int64_t max_steps,
+                                 int64_t log_every, int what, void *stream);
+
+/* Copy up to max_records records out, in the order they were appended (within one segment: unspecified).
+ * *n_records = records copied, *n_dropped (may be NULL) = records lost to the capacity.  Any array pointer may be
+ * NULL.  Always waits for `stream` (the count is a host value).  ESTATE: no log buffer. */
+ENS_API int ens_log_read(const ens_t *e, int64_t *n_records, int64_t *n_dropped, int64_t *sys, int64_t *nsteps,
+                         double *time, int32_t *status, double *pos, double *vel, int64_t max_records, int memspace,
+                         void *stream);
+
 /* Total energy E = sum 1/2 m v^2 - sum_{i<k} m_i m_k / r_ik (Eq. 6, each pair once: R9) and, if
  * L != NULL, total angular momentum sum m x cross v, per system, computed on the device ("only 1-4 values
  * per system need to be transferred").  EINVAL: NULL e or E.  ESTATE: no state was set. */

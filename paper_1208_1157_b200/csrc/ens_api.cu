@@ -155,6 +155,50 @@ __global__ void __launch_bounds__(256) dfma_kernel(int64_t iters, double seed, d
 }
 
 
+// ---------------------------------------------------------------------------------------------------------------
+// State log ("the system's current state is written to a buffer in the GPU global device memory"; reading
+// R-L1/R-L2 of DESIGN.md).  Runs on the stream between two segments of ens_integrate_logged: every system that
+// advanced since its last record (and that the selection asks for) appends one record at an atomic cursor.
+// Record r: sys[r], nsteps[r], time[r], status[r], pos[r][n_body][3], vel[r][n_body][3].  HBM-bound data movement.
+// ---------------------------------------------------------------------------------------------------------------
+struct LogView {
+    int64_t capacity;
+    unsigned long long* cursor;  // [0] = records appended (may exceed capacity: the excess was dropped)
+    int64_t* last;               // [n_pad] nsteps at the last record of each system (-1 = never)
+    int64_t *sys, *nsteps;
+    double* time;
+    int32_t* status;
+    double *pos, *vel;
+};
+
+__global__ void __launch_bounds__(128) log_kernel(ensd::View e, LogView g, int what) {
+    const int64_t sys = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (sys >= e.n_sys) return;
+    const int64_t ns = e.nsteps[sys];
+    if (ns == g.last[sys]) return;  // nothing new since its last record
+    const int st = e.status[sys];
+    const bool stopped = st >= ENS_STOP_CLOSE;
+    if (!((what & ENS_LOG_SNAPSHOTS) || ((what & ENS_LOG_STOPS) && stopped))) return;
+    g.last[sys] = ns;
+    const unsigned long long r = atomicAdd(g.cursor, 1ull);
+    if ((int64_t)r >= g.capacity) return;  // dropped (counted by the cursor)
+    g.sys[r] = sys;
+    g.nsteps[r] = ns;
+    g.time[r] = e.time[sys];
+    g.status[r] = st;
+    const int n3 = e.n_body * 3;
+    for (int k = 0; k < n3; ++k) {
+        g.pos[r * n3 + k] = e.pos[(int64_t)k * e.n_pad + sys];
+        g.vel[r * n3 + k] = e.vel[(int64_t)k * e.n_pad + sys];
+    }
+}
+
+__global__ void log_reset_kernel(int64_t* last, int64_t n, unsigned long long* cursor) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) last[i] = -1;
+    if (i == 0) *cursor = 0ull;
+}
+
 }  // namespace
 
 struct ens {
@@ -174,6 +218,7 @@ struct ens {
     int64_t launches;
     cudaEvent_t ev0, ev1;
     bool timed;
+    LogView log;  // capacity 0 = no log buffer
 };
 
 namespace {
@@ -261,6 +306,14 @@ int ens_destroy(ens_t* e) {
     cudaFree(e->v.status);
     cudaFree(e->v.nsteps);
     cudaFree(e->counter);
+    cudaFree(e->log.cursor);
+    cudaFree(e->log.last);
+    cudaFree(e->log.sys);
+    cudaFree(e->log.nsteps);
+    cudaFree(e->log.time);
+    cudaFree(e->log.status);
+    cudaFree(e->log.pos);
+    cudaFree(e->log.vel);
     ensd::adaptive_order_free(e->order);
     cudaFree(e->stage);
     cudaFree(e->stage_small);
@@ -308,6 +361,8 @@ int ens_set_state(ens_t* e, const double* pos, const double* vel, const double* 
                                                                       e->v.n_pad);
     e->launches += 4;
     CU(cudaGetLastError());
+    if (e->log.capacity)  // step counters restart at 0: forget what was logged (records already taken stay)
+        CU(cudaMemsetAsync(e->log.last, 0xFF, sizeof(int64_t) * e->v.n_pad, s));
     if (memspace == ENS_HOST) CU(cudaStreamSynchronize(s));
     e->have_state = true;
     return ENS_OK;
@@ -414,6 +469,76 @@ int ens_energy(const ens_t* e, double* E, double* L, int memspace, void* stream)
         CU(cudaMemcpyAsync(E, dE, sizeof(double) * n, cudaMemcpyDeviceToHost, s));
         if (L) CU(cudaMemcpyAsync(L, dL, sizeof(double) * n * 3, cudaMemcpyDeviceToHost, s));
         CU(cudaStreamSynchronize(s));
+    }
+    return ENS_OK;
+}
+
+int ens_log_enable(ens_t* e, int64_t capacity, void* stream) {
+    if (!e || capacity < 0) return ENS_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    CU(cudaStreamSynchronize(s));
+    LogView& g = e->log;
+    cudaFree(g.cursor); cudaFree(g.last); cudaFree(g.sys); cudaFree(g.nsteps);
+    cudaFree(g.time); cudaFree(g.status); cudaFree(g.pos); cudaFree(g.vel);
+    memset(&g, 0, sizeof g);
+    if (capacity == 0) return ENS_OK;
+    const int64_t n3 = (int64_t)e->v.n_body * 3;
+    CU(cudaMalloc(&g.cursor, sizeof(unsigned long long)));
+    CU(cudaMalloc(&g.last, sizeof(int64_t) * e->v.n_pad));
+    CU(cudaMalloc(&g.sys, sizeof(int64_t) * capacity));
+    CU(cudaMalloc(&g.nsteps, sizeof(int64_t) * capacity));
+    CU(cudaMalloc(&g.time, sizeof(double) * capacity));
+    CU(cudaMalloc(&g.status, sizeof(int32_t) * capacity));
+    CU(cudaMalloc(&g.pos, sizeof(double) * capacity * n3));
+    CU(cudaMalloc(&g.vel, sizeof(double) * capacity * n3));
+    g.capacity = capacity;
+    log_reset_kernel<<<(unsigned)((e->v.n_pad + 255) / 256), 256, 0, s>>>(g.last, e->v.n_pad, g.cursor);
+    e->launches += 1;
+    CU(cudaGetLastError());
+    return ENS_OK;
+}
+
+int ens_integrate_logged(ens_t* e, int integrator, double dt, double t_end, int64_t max_steps, int64_t log_every,
+                         int what, void* stream) {
+    if (!e || log_every < 1 || !(what & (ENS_LOG_SNAPSHOTS | ENS_LOG_STOPS))) return ENS_EINVAL;
+    if (e->log.capacity == 0) return ENS_ESTATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    int64_t done = 0;
+    do {  // segments of log_every steps, each followed by the log kernel: all enqueued, no host round trip
+        const int64_t seg = (max_steps - done < log_every) ? (max_steps - done) : log_every;
+        const int rc = ens_integrate(e, integrator, dt, t_end, seg, stream);
+        if (rc != ENS_OK) return rc;
+        log_kernel<<<(unsigned)((e->v.n_sys + 127) / 128), 128, 0, s>>>(e->v, e->log, what);
+        e->launches += 1;
+        CU(cudaGetLastError());
+        done += seg;
+    } while (done < max_steps);
+    return ENS_OK;
+}
+
+int ens_log_read(const ens_t* e, int64_t* n_records, int64_t* n_dropped, int64_t* sys, int64_t* nsteps, double* time,
+                 int32_t* status, double* pos, double* vel, int64_t max_records, int memspace, void* stream) {
+    if (!e || !n_records || max_records < 0 || (memspace != ENS_HOST && memspace != ENS_DEVICE)) return ENS_EINVAL;
+    if (e->log.capacity == 0) return ENS_ESTATE;
+    cudaStream_t s = (cudaStream_t)stream;
+    const LogView& g = e->log;
+    unsigned long long cur = 0;
+    CU(cudaMemcpyAsync(&cur, g.cursor, sizeof cur, cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));  // the record count is a host value: this call always waits for the stream
+    const int64_t stored = (int64_t)cur < g.capacity ? (int64_t)cur : g.capacity;
+    const int64_t n = stored < max_records ? stored : max_records;
+    *n_records = n;
+    if (n_dropped) *n_dropped = (int64_t)cur - stored;
+    const cudaMemcpyKind kind = memspace == ENS_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+    const int64_t n3 = (int64_t)e->v.n_body * 3;
+    if (n > 0) {
+        if (sys) CU(cudaMemcpyAsync(sys, g.sys, sizeof(int64_t) * n, kind, s));
+        if (nsteps) CU(cudaMemcpyAsync(nsteps, g.nsteps, sizeof(int64_t) * n, kind, s));
+        if (time) CU(cudaMemcpyAsync(time, g.time, sizeof(double) * n, kind, s));
+        if (status) CU(cudaMemcpyAsync(status, g.status, sizeof(int32_t) * n, kind, s));
+        if (pos) CU(cudaMemcpyAsync(pos, g.pos, sizeof(double) * n * n3, kind, s));
+        if (vel) CU(cudaMemcpyAsync(vel, g.vel, sizeof(double) * n * n3, kind, s));
+        if (memspace == ENS_HOST) CU(cudaStreamSynchronize(s));
     }
     return ENS_OK;
 }

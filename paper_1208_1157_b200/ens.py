@@ -16,6 +16,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE, EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 HERMITE, MVS, HERMITE_ADAPTIVE, HERMITE_CARRY, RKCK = 0, 1, 2, 3, 4  # HERMITE_ADAPTIVE: `dt` is the step size scale tau of Eq. 5
 HOST, DEVICE = 0, 1
 ACTIVE, DONE_TIME, DONE_STEPS, STOP_CLOSE, STOP_EJECT, STOP_NONFINITE = range(6)
+LOG_SNAPSHOTS, LOG_STOPS = 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libens.so")
@@ -23,7 +24,7 @@ LIB_PATH = os.path.join(_HERE, "libens.so")
 SYMBOLS = (
     "ens_create", "ens_destroy", "ens_set_state", "ens_set_monitors", "ens_integrate", "ens_get_state",
     "ens_energy", "ens_strerror", "ens_get_info", "ens_last_kernel_ms", "ens_fp64_peak", "ens_test_rsqrt",
-    "ens_test_rcp",
+    "ens_test_rcp", "ens_log_enable", "ens_integrate_logged", "ens_log_read",
 )
 _lib = None
 
@@ -59,6 +60,9 @@ def lib() -> ctypes.CDLL:
         L.ens_fp64_peak.argtypes = [i64, ctypes.POINTER(cd), vp]
         L.ens_test_rsqrt.argtypes = [vp, vp, i64, vp]
         L.ens_test_rcp.argtypes = [vp, vp, i64, vp]
+        L.ens_log_enable.argtypes = [vp, i64, vp]
+        L.ens_integrate_logged.argtypes = [vp, ci, cd, cd, i64, i64, ci, vp]
+        L.ens_log_read.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64), vp, vp, vp, vp, vp, vp, i64, ci, vp]
         for name in SYMBOLS:
             if name != "ens_strerror":
                 getattr(L, name).restype = ci
@@ -184,6 +188,30 @@ class Ensemble:
             E, L = np.empty(n), np.empty((n, 3))
             _check(lib().ens_energy(self._h, E.ctypes.data, L.ctypes.data, HOST, _stream_ptr(stream)), "ens_energy")
         return E, L
+
+    # -- ens_log_enable / ens_integrate_logged / ens_log_read ------------------------------------------
+    def log_enable(self, capacity: int, stream=None):
+        _check(lib().ens_log_enable(self._h, int(capacity), _stream_ptr(stream)), "ens_log_enable")
+        self._log_capacity = int(capacity)
+
+    def integrate_logged(self, integrator: int, dt: float, max_steps: int, log_every: int, what: int = LOG_SNAPSHOTS,
+                         t_end: float = float("inf"), stream=None):
+        _check(lib().ens_integrate_logged(self._h, int(integrator), float(dt), float(t_end), int(max_steps),
+                                          int(log_every), int(what), _stream_ptr(stream)), "ens_integrate_logged")
+
+    def log_read(self, stream=None):
+        """dict(sys, nsteps, time, status, pos, vel, dropped) of the records appended so far (host arrays)."""
+        cap, nb = self._log_capacity, self.n_body
+        out = dict(sys=np.empty(cap, np.int64), nsteps=np.empty(cap, np.int64), time=np.empty(cap),
+                   status=np.empty(cap, np.int32), pos=np.empty((cap, nb, 3)), vel=np.empty((cap, nb, 3)))
+        n, dropped = ctypes.c_int64(), ctypes.c_int64()
+        _check(lib().ens_log_read(self._h, ctypes.byref(n), ctypes.byref(dropped), out["sys"].ctypes.data,
+                                  out["nsteps"].ctypes.data, out["time"].ctypes.data, out["status"].ctypes.data,
+                                  out["pos"].ctypes.data, out["vel"].ctypes.data, cap, HOST, _stream_ptr(stream)),
+               "ens_log_read")
+        out = {k: v[:n.value] for k, v in out.items()}
+        out["dropped"] = dropped.value
+        return out
 
     # -- helpers ------------------------------------------------------------------------------------
     def info(self) -> dict:
