@@ -12,11 +12,13 @@
 // Layout of every array argument: C order, pos/vel [n_sys][n_body][3], mass [n_sys][n_body], per-system
 // arrays [n_sys].  Body 0 is the central body.  G = 1.
 //
-// Pins (tests/test_oracle_*.py): 2-body closed forms, Kepler's equation, order-4 / order-2 convergence,
-// symmetric-corrector identity, reversal, invariants, finite-difference jerk, brute-force sums, Stumpff
-// closed forms, test-particle exactness of the Kepler drift, hand-built monitor crossings.  No function
-// in this file is "parity unpinned"; the only unpinned item is the paper's Table 1, whose
-// orbital phases are unspecified.
+// Pins (tests/test_oracle_*.py, tests/test_golden.py): 2-body closed forms, Kepler's equation, order-4 / order-2
+// convergence, symmetric-corrector identity, reversal, invariants, finite-difference jerk, brute-force sums, Stumpff
+// closed forms, test-particle exactness of the Kepler drift, hand-built monitor crossings; adaptive step (Eq. 5):
+// circular and apsidal closed forms dt = tau / (w sqrt 2), scaling laws, order 4 in tau; 2-evaluation Hermite: order
+// 4, first step identical to the 3-evaluation step; Cash-Karp: all 17 rooted-tree order conditions on the tableau,
+// measured order 5 (embedded: 4).  No function in this file is "parity unpinned"; the only unpinned item is the
+// paper's Table 1, whose orbital phases are unspecified.
 
 #include <cmath>
 #include <cstdint>
