@@ -146,11 +146,11 @@ ENS_API int ens_last_kernel_ms(const ens_t *e, float *ms);
  * measured denominator of the FP64 roofline (MEASURED_PEAKS.json has no FP64 entry). */
 ENS_API int ens_fp64_peak(int64_t iters, double *lane_fma_per_s, void *stream);
 
-/* Device function test hook: y[i] = the library's FP64 reciprocal square root of x[i] (float rsqrt seed +
+/* Device function test hook: y[i] = the library's FP64 reciprocal square root of x[i] (MUFU.RSQ64H seed +
  * FP64 refinement, P:L276 / R14), device pointers, n elements. */
 ENS_API int ens_test_rsqrt(const double *x, double *y, int64_t n, void *stream);
 
-/* Device function test hook: y[i] = the library's FP64 reciprocal of x[i] (float rcp seed + FP64 refinement; used
+/* Device function test hook: y[i] = the library's FP64 reciprocal of x[i] (MUFU.RCP64H seed + FP64 refinement; used
  * by the MVS Kepler drift instead of the IEEE divide), device pointers, n elements. */
 ENS_API int ens_test_rcp(const double *x, double *y, int64_t n, void *stream);
 

@@ -25,7 +25,7 @@ template <int N> struct ShapeOf;
 #define ENS_H3_MAXT 64  // __launch_bounds__ threads: with MINB it sets the register cap 65536 / (MAXT * MINB)
 #endif
 #ifndef ENS_H3_MINB
-#define ENS_H3_MINB 7  // 128 registers, no spills, 8 blocks of 2 warps per SM: 43.9 ms vs 48.1 ms at 188 registers
+#define ENS_H3_MINB 7  // register cap 128 (125 used, no spills), 8 blocks of 2 warps per SM (sweeps: DESIGN.md §8)
 #endif
 //        N  L  B  unroll threads minBlocks
 ENS_SHAPE(2, 1, 2, true, 64, 1)
