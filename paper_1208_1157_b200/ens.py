@@ -1,7 +1,7 @@
 """Thin ctypes binding over the C ABI of ``include/ens.h`` (``libens.so``).  Same names, argument marshalling only:
 every step of the path runs in the CUDA kernels of ``csrc/``.  torch is used for device memory and streams.
 
-There is NO CPU fallback: if ``libens.so`` is missing the import of the library raises, and every call raises
+There is NO CPU fallback: if ``libens.so`` is missing it is compiled with nvcc on first use, and if that fails the load raises, and every call raises
 ``EnsError`` when the C function returns an error (e.g. no CUDA device).
 """
 from __future__ import annotations
@@ -41,9 +41,16 @@ def lib() -> ctypes.CDLL:
     global _lib
     if _lib is None:
         if not os.path.exists(LIB_PATH):
-            raise ImportError(
-                f"{LIB_PATH} not found: run `python -m paper_1208_1157_b200.build` (nvcc, sm_100a). "
-                "There is no CPU fallback.")
+            # a fresh checkout (the .so is git-ignored): compile it, once, with nvcc; never fall back to anything else
+            try:
+                from . import build as _build
+                if os.path.abspath(LIB_PATH) != os.path.abspath(_build.LIB):
+                    raise RuntimeError("a non-default LIB_PATH is never built implicitly")
+                _build.build()
+            except Exception as ex:
+                raise ImportError(
+                    f"{LIB_PATH} not found and could not be built ({ex}): run `python -m paper_1208_1157_b200.build` "
+                    "(nvcc, sm_100a). There is no CPU fallback.") from ex
         L = ctypes.CDLL(LIB_PATH)
         vp, i64, ci, cd = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double
         L.ens_create.argtypes = [i64, ci, ctypes.POINTER(vp)]
