@@ -44,7 +44,7 @@ ENS_SHAPE(5, 1, 5, false, 64, 1)
 #define ENS_H6_MINB 1
 #endif
 #ifndef ENS_H6_UNROLL
-#define ENS_H6_UNROLL false
+#define ENS_H6_UNROLL true  // straight-line step (three copies of the 15-pair evaluation): 0.668 against 0.653 for the 3-phase loop
 #endif
 ENS_SHAPE_T(6, ENS_H6_L, ENS_H6_B, ENS_H6_UNROLL, ENS_H6_THREADS, ENS_H6_MINB, ENS_H6_MAXT)
 ENS_SHAPE(7, 3, 3, false, 64, 1)
