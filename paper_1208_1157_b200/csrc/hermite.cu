@@ -30,8 +30,8 @@ template <int N> struct ShapeOf;
 //        N  L  B  unroll threads minBlocks
 ENS_SHAPE(2, 1, 2, true, 64, 1)
 ENS_SHAPE_T(3, 1, 3, ENS_H3_UNROLL, ENS_H3_THREADS, ENS_H3_MINB, ENS_H3_MAXT)
-ENS_SHAPE(4, 1, 4, false, 64, 1)
-ENS_SHAPE(5, 1, 5, false, 64, 1)
+ENS_SHAPE(4, 1, 4, true, 64, 1)
+ENS_SHAPE(5, 1, 5, true, 64, 1)
 // n_body = 6 (config 2): one system per thread, all 15 pairs in one lane, no shuffles: 0.62 of FP64 issue peak against
 // 0.54 for the best 3-lane shape; 32-thread blocks spread the 1024 warps of config 2 evenly over the SMs.
 #ifndef ENS_H6_L
