@@ -64,7 +64,10 @@ ENS_SHAPE(14, 5, 3, false, 64, 1)
 #define ENS_H15_MAXT 128
 #define ENS_H15_MINB 1
 #endif
-ENS_SHAPE_T(15, ENS_H15_L, ENS_H15_B, false, ENS_H15_THREADS, ENS_H15_MINB, ENS_H15_MAXT)
+#ifndef ENS_H15_UNROLL
+#define ENS_H15_UNROLL false
+#endif
+ENS_SHAPE_T(15, ENS_H15_L, ENS_H15_B, ENS_H15_UNROLL, ENS_H15_THREADS, ENS_H15_MINB, ENS_H15_MAXT)
 ENS_SHAPE(16, 5, 4, false, 64, 1)
 #undef ENS_SHAPE
 #undef ENS_SHAPE_T

@@ -441,10 +441,13 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 else
                     r2min = p.rc2_bits ? pair_r2min<N, L, B>(X, l, base, amask) : ~0ull;
                 accept_and_predict(amask);
+                // lanes that just stopped take no part in the shuffles of the corrector evaluations
+                unsigned am2 = amask;
+                if constexpr (L > 1) am2 = __ballot_sync(amask, active);
                 if (active) {
-                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, amask);
+                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am2);
                     correct();
-                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, amask);
+                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am2);
                     correct();
                     t += h;
                     ++k;
