@@ -205,7 +205,9 @@ def main():
     c = W.CONFIGS[CFG]
     n_sys, n_body = c.n_sys, c.n_body
     # each rank owns its own range of system indices of the same seeded generator (weak scaling, no exchange)
-    pos, vel, mass = W.generate(CFG, n_sys=n_sys, offset=rank * n_sys)
+    from paper_1208_1157_b200 import shard
+    lo, hi = shard.weak_range(n_sys, rank)
+    pos, vel, mass = W.generate(CFG, n_sys=hi - lo, offset=lo)
     d_pos, d_vel, d_mass = (torch.from_numpy(x).cuda() for x in (pos, vel, mass))
     h_pos, h_vel, h_mass = (torch.from_numpy(x).pin_memory() for x in (pos, vel, mass))
     stream = torch.cuda.Stream()

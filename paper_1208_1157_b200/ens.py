@@ -1,8 +1,8 @@
 """Thin ctypes binding over the C ABI of ``include/ens.h`` (``libens.so``).  Same names, argument marshalling only:
 every step of the path runs in the CUDA kernels of ``csrc/``.  torch is used for device memory and streams.
 
-There is NO CPU fallback: if ``libens.so`` is missing it is compiled with nvcc on first use, and if that fails the load raises, and every call raises
-``EnsError`` when the C function returns an error (e.g. no CUDA device).
+There is NO CPU fallback: if ``libens.so`` is missing it is compiled with nvcc on first use; if that fails the load
+raises, and every call raises ``EnsError`` when the C function returns an error (e.g. no CUDA device).
 """
 from __future__ import annotations
 
