@@ -106,3 +106,31 @@ def test_monitors_split_runs_and_direction():
         e.integrate(ens.HERMITE_ADAPTIVE, -0.02, 10**6, t_end=0.0)
         c = e.get_state()
         assert (c["status"] == ens.DONE_TIME).all() and (c["time"] <= 0.0).all() and (c["time"] > -0.1).all()
+
+
+def test_results_do_not_depend_on_the_hand_out_order_and_stops_are_sticky(monkeypatch):
+    """The longest-first hand-out (adaptive_order.cu) only schedules: with it switched off every system ends in the
+    bit-identical state.  A system stopped by a monitor is not touched by a second call (it is pulled, found stopped,
+    and retired without a write-back)."""
+    pos, vel, mass = W.generate(1, n_sys=3000)
+    pos[11, 2] = pos[11, 1] + np.array([0.05, 0.0, 0.0])
+    vel[11, 2] = vel[11, 1] + np.array([-0.5, 0.0, 0.0])
+    runs = []
+    for unordered in (False, True):
+        if unordered:
+            monkeypatch.setenv("ENS_ADAPTIVE_UNORDERED", "1")
+        with ens.Ensemble(3000, 3) as e:
+            e.set_state(pos, vel, mass)
+            e.set_monitors(0.02, 100.0)
+            e.integrate(ens.HERMITE_ADAPTIVE, 0.03, 10**6, 6.0)
+            a = e.get_state()
+            e.integrate(ens.HERMITE_ADAPTIVE, 0.03, 50)
+            b = e.get_state()
+        assert a["status"][11] == ens.STOP_CLOSE and b["status"][11] == ens.STOP_CLOSE
+        assert (b["pos"][11] == a["pos"][11]).all() and b["nsteps"][11] == a["nsteps"][11] and b["time"][11] == a["time"][11]
+        others = np.arange(3000) != 11
+        assert (b["nsteps"][others] == a["nsteps"][others] + 50).all() and (b["status"][others] == ens.DONE_STEPS).all()
+        runs.append((a, b))
+    for x, y in zip(runs[0], runs[1]):
+        for key in ("pos", "vel", "time", "status", "nsteps"):
+            assert (x[key] == y[key]).all(), key
