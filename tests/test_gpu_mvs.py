@@ -2,6 +2,8 @@
 Tolerance (BASELINE.json north_star, config 4): max relative position/velocity difference <= 1e-10.
 R-noise / DESIGN.md §7: at 10^4 steps the FP64 rounding floor itself (oracle double vs oracle long double) exceeds
 1e-10 for a few systems per thousand, so the 10^4-step comparison is made per system against that system's own floor."""
+import math
+
 import numpy as np
 import pytest
 
@@ -163,3 +165,40 @@ def test_rcp_within_one_ulp():
     err = np.abs((y.astype(np.longdouble) - ref) / np.spacing(np.abs(ref).astype(np.float64))).astype(np.float64)
     print(f"rcp: max error {err.max():.3f} ulp, mean {err.mean():.3f}")
     assert err.max() <= 1.0
+
+
+def test_kepler_drift_stress_against_the_oracle():
+    """The kernel's Kepler solver (Chebyshev-corrected Newton, Taylor finish, series / quartered Stumpff, bisection
+    fallback) against the oracle's plain Newton solver on 3000 random test particles: circular to strongly hyperbolic,
+    steps from a hundredth of a radian to several revolutions, both directions.  With massless planets one MVS step
+    is exactly one Kepler drift of each planet about the unit-mass star (R-M5)."""
+    rng = np.random.default_rng(2024)
+    n_sys, n_pl = 1000, 3
+    pos = np.zeros((n_sys, n_pl + 1, 3))
+    vel = np.zeros((n_sys, n_pl + 1, 3))
+    mass = np.zeros((n_sys, n_pl + 1))
+    mass[:, 0] = 1.0
+    for b in range(1, n_pl + 1):
+        r = 10.0 ** rng.uniform(-0.5, 1.0, n_sys)
+        d = rng.normal(size=(n_sys, 3))
+        d /= np.linalg.norm(d, axis=1)[:, None]
+        pos[:, b] = r[:, None] * d
+        w = rng.normal(size=(n_sys, 3))
+        w /= np.linalg.norm(w, axis=1)[:, None]
+        speed = np.sqrt(1.0 / r) * 10.0 ** rng.uniform(-0.7, 0.35, n_sys)  # 0.2 .. 2.2 of circular: e up to ~4
+        vel[:, b] = speed[:, None] * w
+    for dt in (0.05, 3.0, -11.0, 40.0):
+        g = ens.run(ens.MVS, pos, vel, mass, dt=dt, steps=1, t_end=math.copysign(math.inf, dt))
+        worst = 0.0
+        for s in range(0, n_sys, 7):  # the oracle is called particle by particle: a strided sample
+            for b in range(1, n_pl + 1):
+                # reference: the oracle in long double; tolerance: 1e-11, or 10 x the oracle's own double-vs-long-double
+                # difference where that is larger (a step of 40 spans up to ~60 revolutions of the tightest orbits)
+                q, p, _ = oracle.kepler_drift(pos[s, b], vel[s, b], 1.0, dt, prec=oracle.LONG_DOUBLE)
+                qd, pd, _ = oracle.kepler_drift(pos[s, b], vel[s, b], 1.0, dt)
+                sq, sp = np.linalg.norm(q) + np.linalg.norm(pos[s, b]), np.linalg.norm(p) + np.linalg.norm(vel[s, b])
+                floor = max(np.abs(qd - q).max() / sq, np.abs(pd - p).max() / sp)
+                err = max(np.abs(g["pos"][s, b] - q).max() / sq, np.abs(g["vel"][s, b] - p).max() / sp)
+                worst = max(worst, err / max(1e-11, 10 * floor))
+        assert worst <= 1.0, (dt, worst)
+        assert (g["status"] == ens.DONE_STEPS).all() and (g["nsteps"] == 1).all() and np.isfinite(g["pos"]).all()
