@@ -354,6 +354,59 @@ def main():
                     del pk, vk, mk
                 except ens.EnsError as ex:
                     others[ck.name] = {"unavailable": str(ex)}
+            # HBM side of the path (rows a1 / a8 and the boundary kernels): achieved GB/s against MEASURED_PEAKS.json's
+            # copy bandwidth, on the metric's ensemble and on one 16x larger (small launches are latency-bound)
+            try:
+                with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+                    hbm_peak = float(json.load(f)["hbm_gbs"])
+            except Exception:
+                hbm_peak = None
+            hbm = {"peak_gbs": hbm_peak, "peak_source": "MEASURED_PEAKS.json hbm_gbs" if hbm_peak else "unavailable"}
+            for tag, ns in (("131072x3", n_sys), ("2097152x3", 16 * n_sys)):
+                try:
+                    pk, vk, mk = (torch.from_numpy(x).cuda() for x in W.generate(CFG, n_sys=ns, offset=lo))
+                    ek = ens.Ensemble(ns, n_body)
+                    outk = {"pos": torch.empty_like(pk), "vel": torch.empty_like(vk),
+                            "time": torch.empty(ns, dtype=torch.float64, device="cuda"),
+                            "status": torch.empty(ns, dtype=torch.int32, device="cuda"),
+                            "nsteps": torch.empty(ns, dtype=torch.int64, device="cuda")}
+                    Ek = torch.empty(ns, dtype=torch.float64, device="cuda")
+
+                    def timed(fn, reps=5):
+                        best = None
+                        for _ in range(reps):
+                            flush.zero_()
+                            t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                            t0.record(stream)
+                            fn()
+                            t1.record(stream)
+                            t1.synchronize()
+                            best = t0.elapsed_time(t1) if best is None else min(best, t0.elapsed_time(t1))
+                        return best * 1e-3
+
+                    nb8 = n_body * 8
+                    legs = {
+                        # AoS read + SoA write of pos, vel, mass, plus the time/status/nsteps reset
+                        "set_state": (lambda: ek.set_state(pk, vk, mk, stream=stream), ns * (2 * 7 * nb8 + 20)),
+                        # zero steps: every row read once and written once by the step-loop kernel (a1 + a8)
+                        "integrate_0_steps": (lambda: ek.integrate(ens.HERMITE, c.dt, 0, stream=stream),
+                                              ns * ((13 * n_body + 2) * 8 + 12)),
+                        "get_state": (lambda: ek.get_state(stream=stream, out=outk), ns * (2 * 6 * nb8 + 2 * 20)),
+                        "energy": (lambda: ens._check(ens.lib().ens_energy(ek._h, Ek.data_ptr(), None, ens.DEVICE,
+                                                                          stream.cuda_stream), "ens_energy"),
+                                   ns * (7 * nb8 + 8)),
+                    }
+                    ek.set_state(pk, vk, mk, stream=stream)
+                    hbm[tag] = {}
+                    for name, (fn, nbytes) in legs.items():
+                        sec = timed(fn)
+                        hbm[tag][name] = {"us": sec * 1e6, "gbs": nbytes / sec / 1e9,
+                                          "frac": (nbytes / sec / 1e9 / hbm_peak) if hbm_peak else None}
+                    ek.close()
+                    del pk, vk, mk, outk, Ek
+                except ens.EnsError as ex:
+                    hbm[tag] = {"unavailable": str(ex)}
+            line["hbm"] = hbm
             # adaptive-step Hermite (Eq. 5) on the metric's own systems, tau = 0.017 to t = 20; event-timed
             # around the C-ABI call (ordering pre-pass + kernel); system-steps = steps actually taken
             try:

@@ -29,15 +29,15 @@ constexpr int TILE = 64;  // systems per transposition tile = padding granule of
 
 // ---------------------------------------------------------------------------------------------------------------
 // AoS [n_sys][K] <-> SoA [K][n_pad] transposition through shared memory, 128-bit global accesses on both sides
-// (north_star item 2).  One block per tile of 64 systems; K = 3 n_body (pos, vel) or n_body (mass).
-// Pure data movement: HBM-bound, 16 bytes of traffic per double.
+// (north_star item 2).  One block per tile of 64 systems; K = 3 n_body (pos, vel) or n_body (mass) is a compile-time
+// constant (the index arithmetic of a run-time K made these kernels ALU-bound).  ens_set_state is ONE launch: pos, vel
+// and mass tiles one after the other through the same shared buffer, then the time / status / nsteps reset of the
+// tile's systems.  Pure data movement: HBM-bound, 16 bytes of traffic per double.
 // ---------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) pack_kernel(const double* __restrict__ src, double* __restrict__ dst,
-                                                   int64_t n_sys, int64_t n_pad, int K, int vec_ok) {
-    extern __shared__ double tile[];  // [TILE][Kp], Kp odd: conflict-free column reads
-    const int Kp = K | 1;
-    const int64_t sys0 = (int64_t)blockIdx.x * TILE;
-    const int nv = (int)((n_sys - sys0 < TILE) ? (n_sys - sys0) : TILE);
+template <int K>
+__device__ __forceinline__ void pack_tile(const double* __restrict__ src, double* __restrict__ dst, double* tile,
+                                          int64_t sys0, int nv, int64_t n_pad, bool vec_ok) {
+    constexpr int Kp = K | 1;  // odd pitch: conflict-free column reads
     const int total = nv * K;
     const double* s = src + sys0 * K;
     if (vec_ok && (total & 1) == 0) {
@@ -60,14 +60,13 @@ __global__ void __launch_bounds__(256) pack_kernel(const double* __restrict__ sr
         w.y = sp + 1 < nv ? tile[(sp + 1) * Kp + k] : 0.0;
         *reinterpret_cast<double2*>(dst + (int64_t)k * n_pad + sys0 + sp) = w;
     }
+    __syncthreads();
 }
 
-__global__ void __launch_bounds__(256) unpack_kernel(const double* __restrict__ src, double* __restrict__ dst,
-                                                     int64_t n_sys, int64_t n_pad, int K, int vec_ok) {
-    extern __shared__ double tile[];
-    const int Kp = K | 1;
-    const int64_t sys0 = (int64_t)blockIdx.x * TILE;
-    const int nv = (int)((n_sys - sys0 < TILE) ? (n_sys - sys0) : TILE);
+template <int K>
+__device__ __forceinline__ void unpack_tile(const double* __restrict__ src, double* __restrict__ dst, double* tile,
+                                            int64_t sys0, int nv, int64_t n_pad, bool vec_ok) {
+    constexpr int Kp = K | 1;
     for (int i = threadIdx.x; i < K * (TILE / 2); i += blockDim.x) {
         const int k = i / (TILE / 2), sp = (i % (TILE / 2)) * 2;
         const double2 w = *reinterpret_cast<const double2*>(src + (int64_t)k * n_pad + sys0 + sp);
@@ -89,15 +88,66 @@ __global__ void __launch_bounds__(256) unpack_kernel(const double* __restrict__ 
     } else {
         for (int i = threadIdx.x; i < total; i += blockDim.x) d[i] = tile[(i / K) * Kp + (i % K)];
     }
+    __syncthreads();
 }
 
-__global__ void reset_kernel(double* time, int32_t* status, int64_t* nsteps, const double* time_src, int64_t n_sys,
-                             int64_t n_pad) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n_pad) return;
-    time[i] = (i < n_sys && time_src) ? time_src[i] : 0.0;
-    status[i] = ENS_ACTIVE;
-    nsteps[i] = 0;
+template <int NB>
+__global__ void __launch_bounds__(256) pack_state_kernel(const double* __restrict__ pos, const double* __restrict__ vel,
+                                                         const double* __restrict__ mass,
+                                                         const double* __restrict__ time_src, ensd::View e,
+                                                         int vec_pos, int vec_vel, int vec_mass) {
+    __shared__ double tile[TILE * ((3 * NB) | 1)];
+    const int64_t sys0 = (int64_t)blockIdx.x * TILE;
+    const int nv = (int)((e.n_sys - sys0 < TILE) ? (e.n_sys - sys0) : TILE);
+    pack_tile<3 * NB>(pos, e.pos, tile, sys0, nv, e.n_pad, vec_pos);
+    pack_tile<3 * NB>(vel, e.vel, tile, sys0, nv, e.n_pad, vec_vel);
+    pack_tile<NB>(mass, e.mass, tile, sys0, nv, e.n_pad, vec_mass);
+    if (threadIdx.x < TILE) {  // resets the padding systems of the last tile too
+        const int64_t i = sys0 + threadIdx.x;
+        e.time[i] = (threadIdx.x < nv && time_src) ? time_src[i] : 0.0;
+        e.status[i] = ENS_ACTIVE;
+        e.nsteps[i] = 0;
+    }
+}
+
+// pos and / or vel (a NULL destination is skipped)
+template <int NB>
+__global__ void __launch_bounds__(256) unpack_state_kernel(ensd::View e, double* __restrict__ pos,
+                                                           double* __restrict__ vel, int vec_pos, int vec_vel) {
+    __shared__ double tile[TILE * ((3 * NB) | 1)];
+    const int64_t sys0 = (int64_t)blockIdx.x * TILE;
+    const int nv = (int)((e.n_sys - sys0 < TILE) ? (e.n_sys - sys0) : TILE);
+    if (pos) unpack_tile<3 * NB>(e.pos, pos, tile, sys0, nv, e.n_pad, vec_pos);
+    if (vel) unpack_tile<3 * NB>(e.vel, vel, tile, sys0, nv, e.n_pad, vec_vel);
+}
+
+#define ENS_FOR_EACH_NB(X) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
+
+cudaError_t launch_pack(const double* pos, const double* vel, const double* mass, const double* time_src,
+                        const ensd::View& v, cudaStream_t s) {
+    const unsigned g = (unsigned)(v.n_pad / TILE);
+    auto al = [](const void* p) { return (int)((reinterpret_cast<uintptr_t>(p) & 15) == 0); };
+    switch (v.n_body) {
+#define X(N_) \
+    case N_: pack_state_kernel<N_><<<g, 256, 0, s>>>(pos, vel, mass, time_src, v, al(pos), al(vel), al(mass)); break;
+        ENS_FOR_EACH_NB(X)
+#undef X
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_unpack(const ensd::View& v, double* pos, double* vel, cudaStream_t s) {
+    const unsigned g = (unsigned)(v.n_pad / TILE);
+    auto al = [](const void* p) { return (int)((reinterpret_cast<uintptr_t>(p) & 15) == 0); };
+    switch (v.n_body) {
+#define X(N_) \
+    case N_: unpack_state_kernel<N_><<<g, 256, 0, s>>>(v, pos, vel, al(pos), al(vel)); break;
+        ENS_FOR_EACH_NB(X)
+#undef X
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -230,9 +280,6 @@ int ensure_stage(ens* e) {
     return ENS_OK;
 }
 
-int64_t tiles(const ens* e) { return e->v.n_pad / TILE; }
-size_t tile_smem(int K) { return sizeof(double) * TILE * (size_t)(K | 1); }
-int aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
 }  // namespace
 
@@ -352,15 +399,8 @@ int ens_set_state(ens_t* e, const double* pos, const double* vel, const double* 
             dtime = e->stage_small;
         }
     }
-    const int K3 = (int)nb * 3, K1 = (int)nb;
-    const unsigned g = (unsigned)tiles(e);
-    pack_kernel<<<g, 256, tile_smem(K3), s>>>(dpos, e->v.pos, n, e->v.n_pad, K3, aligned16(dpos));
-    pack_kernel<<<g, 256, tile_smem(K3), s>>>(dvel, e->v.vel, n, e->v.n_pad, K3, aligned16(dvel));
-    pack_kernel<<<g, 256, tile_smem(K1), s>>>(dmass, e->v.mass, n, e->v.n_pad, K1, aligned16(dmass));
-    reset_kernel<<<(unsigned)((e->v.n_pad + 255) / 256), 256, 0, s>>>(e->v.time, e->v.status, e->v.nsteps, dtime, n,
-                                                                      e->v.n_pad);
-    e->launches += 4;
-    CU(cudaGetLastError());
+    CU(launch_pack(dpos, dvel, dmass, dtime, e->v, s));
+    e->launches += 1;
     if (e->log.capacity)  // step counters restart at 0: forget what was logged (records already taken stay)
         CU(cudaMemsetAsync(e->log.last, 0xFF, sizeof(int64_t) * e->v.n_pad, s));
     if (memspace == ENS_HOST) CU(cudaStreamSynchronize(s));
@@ -422,24 +462,20 @@ int ens_get_state(const ens_t* e, double* pos, double* vel, double* time, int32_
     ens* me = const_cast<ens*>(e);
     cudaStream_t s = (cudaStream_t)stream;
     const int64_t n = e->v.n_sys, nb = e->v.n_body;
-    const int K3 = (int)nb * 3;
-    const unsigned g = (unsigned)tiles(e);
     const cudaMemcpyKind kind = memspace == ENS_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
     if (memspace == ENS_HOST && (pos || vel)) {
         const int rc = ensure_stage(me);
         if (rc) return rc;
     }
-    if (pos) {
-        double* d = memspace == ENS_HOST ? e->stage : pos;
-        unpack_kernel<<<g, 256, tile_smem(K3), s>>>(e->v.pos, d, n, e->v.n_pad, K3, aligned16(d));
+    if (pos || vel) {  // one launch for both
+        double* dp = !pos ? nullptr : memspace == ENS_HOST ? e->stage : pos;
+        double* dv = !vel ? nullptr : memspace == ENS_HOST ? e->stage + n * nb * 3 : vel;
+        CU(launch_unpack(e->v, dp, dv, s));
         me->launches += 1;
-        if (memspace == ENS_HOST) CU(cudaMemcpyAsync(pos, d, sizeof(double) * n * nb * 3, kind, s));
-    }
-    if (vel) {
-        double* d = memspace == ENS_HOST ? e->stage + n * nb * 3 : vel;
-        unpack_kernel<<<g, 256, tile_smem(K3), s>>>(e->v.vel, d, n, e->v.n_pad, K3, aligned16(d));
-        me->launches += 1;
-        if (memspace == ENS_HOST) CU(cudaMemcpyAsync(vel, d, sizeof(double) * n * nb * 3, kind, s));
+        if (memspace == ENS_HOST) {
+            if (pos) CU(cudaMemcpyAsync(pos, dp, sizeof(double) * n * nb * 3, kind, s));
+            if (vel) CU(cudaMemcpyAsync(vel, dv, sizeof(double) * n * nb * 3, kind, s));
+        }
     }
     if (time) CU(cudaMemcpyAsync(time, e->v.time, sizeof(double) * n, kind, s));
     if (status) CU(cudaMemcpyAsync(status, e->v.status, sizeof(int32_t) * n, kind, s));
