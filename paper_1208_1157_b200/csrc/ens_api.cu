@@ -34,14 +34,16 @@ constexpr int TILE = 64;  // systems per transposition tile = padding granule of
 // and mass tiles one after the other through the same shared buffer, then the time / status / nsteps reset of the
 // tile's systems.  Pure data movement: HBM-bound, 16 bytes of traffic per double.
 // ---------------------------------------------------------------------------------------------------------------
+// the four halves of a transposition; the callers place the __syncthreads between a load and its store
 template <int K>
-__device__ __forceinline__ void pack_tile(const double* __restrict__ src, double* __restrict__ dst, double* tile,
-                                          int64_t sys0, int nv, int64_t n_pad, bool vec_ok) {
-    constexpr int Kp = K | 1;  // odd pitch: conflict-free column reads
+__device__ __forceinline__ void aos_to_tile(const double* __restrict__ src, double* tile, int64_t sys0, int nv,
+                                            bool vec_ok) {
+    constexpr int Kp = K | 1;  // odd pitch: conflict-free column accesses
     const int total = nv * K;
     const double* s = src + sys0 * K;
     if (vec_ok && (total & 1) == 0) {
         const double2* s2 = reinterpret_cast<const double2*>(s);
+#pragma unroll 2
         for (int i = threadIdx.x; i < total / 2; i += blockDim.x) {
             const double2 w = s2[i];
             const int i0 = 2 * i, i1 = 2 * i + 1;
@@ -51,7 +53,12 @@ __device__ __forceinline__ void pack_tile(const double* __restrict__ src, double
     } else {
         for (int i = threadIdx.x; i < total; i += blockDim.x) tile[(i / K) * Kp + (i % K)] = s[i];
     }
-    __syncthreads();
+}
+
+template <int K>
+__device__ __forceinline__ void tile_to_soa(const double* tile, double* __restrict__ dst, int64_t sys0, int nv,
+                                            int64_t n_pad) {
+    constexpr int Kp = K | 1;
     // rows of the SoA: two consecutive systems per thread (sys0 and n_pad are multiples of 64: 16-byte aligned)
     for (int i = threadIdx.x; i < K * (TILE / 2); i += blockDim.x) {
         const int k = i / (TILE / 2), sp = (i % (TILE / 2)) * 2;
@@ -60,20 +67,24 @@ __device__ __forceinline__ void pack_tile(const double* __restrict__ src, double
         w.y = sp + 1 < nv ? tile[(sp + 1) * Kp + k] : 0.0;
         *reinterpret_cast<double2*>(dst + (int64_t)k * n_pad + sys0 + sp) = w;
     }
-    __syncthreads();
 }
 
 template <int K>
-__device__ __forceinline__ void unpack_tile(const double* __restrict__ src, double* __restrict__ dst, double* tile,
-                                            int64_t sys0, int nv, int64_t n_pad, bool vec_ok) {
+__device__ __forceinline__ void soa_to_tile(const double* __restrict__ src, double* tile, int64_t sys0, int64_t n_pad) {
     constexpr int Kp = K | 1;
+#pragma unroll 2
     for (int i = threadIdx.x; i < K * (TILE / 2); i += blockDim.x) {
         const int k = i / (TILE / 2), sp = (i % (TILE / 2)) * 2;
         const double2 w = *reinterpret_cast<const double2*>(src + (int64_t)k * n_pad + sys0 + sp);
         tile[sp * Kp + k] = w.x;
         tile[(sp + 1) * Kp + k] = w.y;
     }
-    __syncthreads();
+}
+
+template <int K>
+__device__ __forceinline__ void tile_to_aos(const double* tile, double* __restrict__ dst, int64_t sys0, int nv,
+                                            bool vec_ok) {
+    constexpr int Kp = K | 1;
     const int total = nv * K;
     double* d = dst + sys0 * K;
     if (vec_ok && (total & 1) == 0) {
@@ -88,20 +99,41 @@ __device__ __forceinline__ void unpack_tile(const double* __restrict__ src, doub
     } else {
         for (int i = threadIdx.x; i < total; i += blockDim.x) d[i] = tile[(i / K) * Kp + (i % K)];
     }
-    __syncthreads();
 }
 
+// pos, vel and mass tiles are in flight together (three shared buffers, one barrier) when they fit 48 KB, else one
+// after the other through one buffer
 template <int NB>
 __global__ void __launch_bounds__(256) pack_state_kernel(const double* __restrict__ pos, const double* __restrict__ vel,
                                                          const double* __restrict__ mass,
                                                          const double* __restrict__ time_src, ensd::View e,
                                                          int vec_pos, int vec_vel, int vec_mass) {
-    __shared__ double tile[TILE * ((3 * NB) | 1)];
+    constexpr int T3 = TILE * ((3 * NB) | 1), T1 = TILE * (NB | 1);
+    constexpr bool TOGETHER = (2 * T3 + T1) * sizeof(double) <= 48 * 1024;
+    __shared__ double tile[TOGETHER ? 2 * T3 + T1 : T3];
     const int64_t sys0 = (int64_t)blockIdx.x * TILE;
     const int nv = (int)((e.n_sys - sys0 < TILE) ? (e.n_sys - sys0) : TILE);
-    pack_tile<3 * NB>(pos, e.pos, tile, sys0, nv, e.n_pad, vec_pos);
-    pack_tile<3 * NB>(vel, e.vel, tile, sys0, nv, e.n_pad, vec_vel);
-    pack_tile<NB>(mass, e.mass, tile, sys0, nv, e.n_pad, vec_mass);
+    if constexpr (TOGETHER) {
+        aos_to_tile<3 * NB>(pos, tile, sys0, nv, vec_pos);
+        aos_to_tile<3 * NB>(vel, tile + T3, sys0, nv, vec_vel);
+        aos_to_tile<NB>(mass, tile + 2 * T3, sys0, nv, vec_mass);
+        __syncthreads();
+        tile_to_soa<3 * NB>(tile, e.pos, sys0, nv, e.n_pad);
+        tile_to_soa<3 * NB>(tile + T3, e.vel, sys0, nv, e.n_pad);
+        tile_to_soa<NB>(tile + 2 * T3, e.mass, sys0, nv, e.n_pad);
+    } else {
+        aos_to_tile<3 * NB>(pos, tile, sys0, nv, vec_pos);
+        __syncthreads();
+        tile_to_soa<3 * NB>(tile, e.pos, sys0, nv, e.n_pad);
+        __syncthreads();
+        aos_to_tile<3 * NB>(vel, tile, sys0, nv, vec_vel);
+        __syncthreads();
+        tile_to_soa<3 * NB>(tile, e.vel, sys0, nv, e.n_pad);
+        __syncthreads();
+        aos_to_tile<NB>(mass, tile, sys0, nv, vec_mass);
+        __syncthreads();
+        tile_to_soa<NB>(tile, e.mass, sys0, nv, e.n_pad);
+    }
     if (threadIdx.x < TILE) {  // resets the padding systems of the last tile too
         const int64_t i = sys0 + threadIdx.x;
         e.time[i] = (threadIdx.x < nv && time_src) ? time_src[i] : 0.0;
@@ -110,15 +142,42 @@ __global__ void __launch_bounds__(256) pack_state_kernel(const double* __restric
     }
 }
 
-// pos and / or vel (a NULL destination is skipped)
+// pos and / or vel (a NULL destination is skipped), plus the per-system rows time / status / nsteps (NULL: skipped)
 template <int NB>
 __global__ void __launch_bounds__(256) unpack_state_kernel(ensd::View e, double* __restrict__ pos,
-                                                           double* __restrict__ vel, int vec_pos, int vec_vel) {
-    __shared__ double tile[TILE * ((3 * NB) | 1)];
+                                                           double* __restrict__ vel, double* __restrict__ time,
+                                                           int32_t* __restrict__ status, int64_t* __restrict__ nsteps,
+                                                           int vec_pos, int vec_vel) {
+    constexpr int T3 = TILE * ((3 * NB) | 1);
+    constexpr bool TOGETHER = 2 * T3 * sizeof(double) <= 48 * 1024;
+    __shared__ double tile[TOGETHER ? 2 * T3 : T3];
     const int64_t sys0 = (int64_t)blockIdx.x * TILE;
     const int nv = (int)((e.n_sys - sys0 < TILE) ? (e.n_sys - sys0) : TILE);
-    if (pos) unpack_tile<3 * NB>(e.pos, pos, tile, sys0, nv, e.n_pad, vec_pos);
-    if (vel) unpack_tile<3 * NB>(e.vel, vel, tile, sys0, nv, e.n_pad, vec_vel);
+    if (threadIdx.x < nv) {
+        const int64_t i = sys0 + threadIdx.x;
+        if (time) time[i] = e.time[i];
+        if (status) status[i] = e.status[i];
+        if (nsteps) nsteps[i] = e.nsteps[i];
+    }
+    if (TOGETHER && pos && vel) {
+        soa_to_tile<3 * NB>(e.pos, tile, sys0, e.n_pad);
+        soa_to_tile<3 * NB>(e.vel, tile + (TOGETHER ? T3 : 0), sys0, e.n_pad);
+        __syncthreads();
+        tile_to_aos<3 * NB>(tile, pos, sys0, nv, vec_pos);
+        tile_to_aos<3 * NB>(tile + (TOGETHER ? T3 : 0), vel, sys0, nv, vec_vel);
+    } else {
+        if (pos) {
+            soa_to_tile<3 * NB>(e.pos, tile, sys0, e.n_pad);
+            __syncthreads();
+            tile_to_aos<3 * NB>(tile, pos, sys0, nv, vec_pos);
+            __syncthreads();
+        }
+        if (vel) {
+            soa_to_tile<3 * NB>(e.vel, tile, sys0, e.n_pad);
+            __syncthreads();
+            tile_to_aos<3 * NB>(tile, vel, sys0, nv, vec_vel);
+        }
+    }
 }
 
 #define ENS_FOR_EACH_NB(X) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
@@ -137,12 +196,13 @@ cudaError_t launch_pack(const double* pos, const double* vel, const double* mass
     return cudaGetLastError();
 }
 
-cudaError_t launch_unpack(const ensd::View& v, double* pos, double* vel, cudaStream_t s) {
+cudaError_t launch_unpack(const ensd::View& v, double* pos, double* vel, double* time, int32_t* status,
+                          int64_t* nsteps, cudaStream_t s) {
     const unsigned g = (unsigned)(v.n_pad / TILE);
     auto al = [](const void* p) { return (int)((reinterpret_cast<uintptr_t>(p) & 15) == 0); };
     switch (v.n_body) {
 #define X(N_) \
-    case N_: unpack_state_kernel<N_><<<g, 256, 0, s>>>(v, pos, vel, al(pos), al(vel)); break;
+    case N_: unpack_state_kernel<N_><<<g, 256, 0, s>>>(v, pos, vel, time, status, nsteps, al(pos), al(vel)); break;
         ENS_FOR_EACH_NB(X)
 #undef X
         default: return cudaErrorInvalidValue;
@@ -467,19 +527,22 @@ int ens_get_state(const ens_t* e, double* pos, double* vel, double* time, int32_
         const int rc = ensure_stage(me);
         if (rc) return rc;
     }
-    if (pos || vel) {  // one launch for both
-        double* dp = !pos ? nullptr : memspace == ENS_HOST ? e->stage : pos;
-        double* dv = !vel ? nullptr : memspace == ENS_HOST ? e->stage + n * nb * 3 : vel;
-        CU(launch_unpack(e->v, dp, dv, s));
+    const bool dev = memspace == ENS_DEVICE;
+    if (pos || vel || (dev && (time || status || nsteps))) {  // one launch
+        double* dp = !pos ? nullptr : dev ? pos : e->stage;
+        double* dv = !vel ? nullptr : dev ? vel : e->stage + n * nb * 3;
+        CU(launch_unpack(e->v, dp, dv, dev ? time : nullptr, dev ? status : nullptr, dev ? nsteps : nullptr, s));
         me->launches += 1;
-        if (memspace == ENS_HOST) {
+        if (!dev) {
             if (pos) CU(cudaMemcpyAsync(pos, dp, sizeof(double) * n * nb * 3, kind, s));
             if (vel) CU(cudaMemcpyAsync(vel, dv, sizeof(double) * n * nb * 3, kind, s));
         }
     }
-    if (time) CU(cudaMemcpyAsync(time, e->v.time, sizeof(double) * n, kind, s));
-    if (status) CU(cudaMemcpyAsync(status, e->v.status, sizeof(int32_t) * n, kind, s));
-    if (nsteps) CU(cudaMemcpyAsync(nsteps, e->v.nsteps, sizeof(int64_t) * n, kind, s));
+    if (!dev) {  // the per-system rows are contiguous in the SoA: straight copies
+        if (time) CU(cudaMemcpyAsync(time, e->v.time, sizeof(double) * n, kind, s));
+        if (status) CU(cudaMemcpyAsync(status, e->v.status, sizeof(int32_t) * n, kind, s));
+        if (nsteps) CU(cudaMemcpyAsync(nsteps, e->v.nsteps, sizeof(int64_t) * n, kind, s));
+    }
     CU(cudaGetLastError());
     if (memspace == ENS_HOST) CU(cudaStreamSynchronize(s));
     return ENS_OK;
