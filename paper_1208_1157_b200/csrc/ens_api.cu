@@ -214,14 +214,16 @@ cudaError_t launch_unpack(const ensd::View& v, double* pos, double* vel, double*
 // Energy and angular momentum, Eq. 6 with each unordered pair once (R9).  One thread per system reading
 // the SoA rows (coalesced); correctly rounded sqrt and divide.  HBM-bound: (7 n_body + 4) * 8 bytes per system.
 // ---------------------------------------------------------------------------------------------------------------
+template <int NB>
 __global__ void __launch_bounds__(128) energy_kernel(ensd::View e, double* __restrict__ E, double* __restrict__ Lout) {
     const int64_t sys = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (sys >= e.n_sys) return;
-    const int n = e.n_body;
-    double x[16][3], m[16];
+    double x[NB][3], m[NB];  // compile-time body count: registers, not local memory
     double ke = 0.0, pe = 0.0, L[3] = {0.0, 0.0, 0.0};
-    for (int i = 0; i < n; ++i) {
+#pragma unroll
+    for (int i = 0; i < NB; ++i) {
         double v[3];
+#pragma unroll
         for (int c = 0; c < 3; ++c) {
             x[i][c] = e.pos[(int64_t)(i * 3 + c) * e.n_pad + sys];
             v[c] = e.vel[(int64_t)(i * 3 + c) * e.n_pad + sys];
@@ -232,8 +234,10 @@ __global__ void __launch_bounds__(128) energy_kernel(ensd::View e, double* __res
         L[1] += m[i] * (x[i][2] * v[0] - x[i][0] * v[2]);
         L[2] += m[i] * (x[i][0] * v[1] - x[i][1] * v[0]);
     }
-    for (int i = 0; i < n; ++i)
-        for (int k = i + 1; k < n; ++k) {
+#pragma unroll
+    for (int i = 0; i < NB; ++i)
+#pragma unroll
+        for (int k = i + 1; k < NB; ++k) {
             const double dx = x[k][0] - x[i][0], dy = x[k][1] - x[i][1], dz = x[k][2] - x[i][2];
             pe -= m[i] * m[k] / sqrt(dx * dx + dy * dy + dz * dz);
         }
@@ -561,7 +565,12 @@ int ens_energy(const ens_t* e, double* E, double* L, int memspace, void* stream)
         dE = e->stage_small;
         dL = L ? e->stage_small + n : nullptr;
     }
-    energy_kernel<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(e->v, dE, dL);
+    switch (e->v.n_body) {
+#define X(N_) \
+    case N_: energy_kernel<N_><<<(unsigned)((n + 127) / 128), 128, 0, s>>>(e->v, dE, dL); break;
+        ENS_FOR_EACH_NB(X)
+#undef X
+    }
     me->launches += 1;
     CU(cudaGetLastError());
     if (memspace == ENS_HOST) {
