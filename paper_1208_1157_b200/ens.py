@@ -118,12 +118,13 @@ class Ensemble:
     def __init__(self, n_sys: int, n_body: int):
         self.n_sys, self.n_body = int(n_sys), int(n_body)
         h = ctypes.c_void_p()
-        _check(lib().ens_create(self.n_sys, self.n_body, ctypes.byref(h)), "ens_create")
+        self._lib = lib()  # kept on the instance: module globals may already be gone when __del__ runs at exit
+        _check(self._lib.ens_create(self.n_sys, self.n_body, ctypes.byref(h)), "ens_create")
         self._h = h
 
     def close(self):
         if getattr(self, "_h", None):
-            lib().ens_destroy(self._h)
+            self._lib.ens_destroy(self._h)
             self._h = None
 
     __del__ = close
