@@ -15,8 +15,13 @@
  *     call's work on `stream` has run.
  *   - The handle owns its internal structure-of-arrays device buffers (layout: DESIGN.md §5).
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-space calls only
- *     enqueue work and return.  Host-space calls enqueue the copies on `stream` and then wait for it, so the
- *     host buffers are complete (get) or reusable (set) on return.
+ *     enqueue work and return: they never allocate (ens_create allocates everything ens_integrate needs).
+ *     Host-space calls enqueue the copies on `stream` and then wait for it, so the host buffers are complete (get)
+ *     or reusable (set) on return; the first one also allocates the device staging area, unless
+ *     ens_reserve_host_staging did so before.
+ *   - Every call runs on the CUDA device that was current when the handle was created, whatever device is current
+ *     in the calling thread, and leaves the caller's current device unchanged.  Pointers and streams passed to a
+ *     call must belong to that device.
  *   - Body 0 is the central body.  G = 1.  No softening.
  *   - There is no CPU fallback: without a CUDA device every compute call returns ENS_ECUDA.
  */
@@ -58,6 +63,10 @@ ENS_API int ens_create(int64_t n_sys, int n_body, ens_t **out);
 
 /* Free the handle and its buffers (synchronises the device first).  NULL is a no-op returning ENS_OK. */
 ENS_API int ens_destroy(ens_t *e);
+
+/* Allocate the device staging area the host-space calls copy through (n_sys * (7 n_body + 4) doubles) now instead
+ * of inside the first host-space call.  Idempotent.  EINVAL: NULL handle.  ENOMEM. */
+ENS_API int ens_reserve_host_staging(ens_t *e);
 
 /* Load the state of every system (Alg. 1 "load initial configuration onto the GPU"; the only
  * bulk host->device transfer).  time == NULL means t = 0 for all.  Resets status to ACTIVE and
@@ -153,6 +162,18 @@ ENS_API int ens_test_rsqrt(const double *x, double *y, int64_t n, void *stream);
 /* Device function test hook: y[i] = the library's FP64 reciprocal of x[i] (MUFU.RCP64H seed + FP64 refinement; used
  * by the MVS Kepler drift instead of the IEEE divide), device pointers, n elements. */
 ENS_API int ens_test_rcp(const double *x, double *y, int64_t n, void *stream);
+
+/* Test / measurement hook: override a launch-time choice of the library for this handle (value 0 = back to the
+ * library's default).  Results never depend on these (tests/test_gpu_hermite.py checks bit-identity); they exist for
+ * the sweeps recorded in DESIGN.md section 8.  EINVAL: NULL handle, unknown option, value out of range. */
+enum {
+    ENS_OPT_THREADS = 0,            /* threads per block of the step-loop kernels (multiple of 32, <= the kernel's bound) */
+    ENS_OPT_ADAPTIVE_UNORDERED = 1, /* 1: adaptive kernels hand systems out in index order (no longest-first pre-pass) */
+    ENS_OPT_SLICE_MODE = 2,         /* fixed-step Hermite: 0 library decides, 1 always time-sliced grid, 2 never */
+    ENS_OPT_SLICE_STEPS = 3,        /* steps per time slice */
+    ENS_OPT_SLICE_WARPS_PER_SM = 4  /* persistent warps per SM of the time-sliced grid (<= what fits) */
+};
+ENS_API int ens_test_set_option(ens_t *e, int option, int64_t value);
 
 #ifdef __cplusplus
 }

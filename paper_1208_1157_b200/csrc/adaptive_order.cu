@@ -59,19 +59,26 @@ __global__ void __launch_bounds__(128) order_key_kernel(View e, double t_end, fl
 
 }  // namespace
 
+// All buffers of the hand-out order for n systems (called by ens_create, so that ens_integrate never allocates).  On any
+// failure everything is released again: `ob` is either complete or empty.
+cudaError_t adaptive_order_alloc(int64_t n_sys, OrderBuffers& ob) {
+    const int n = (int)n_sys;
+    cudaError_t err = cudaSuccess;
+    if ((err = cudaMalloc(&ob.key_in, sizeof(float) * n)) == cudaSuccess &&
+        (err = cudaMalloc(&ob.key_out, sizeof(float) * n)) == cudaSuccess &&
+        (err = cudaMalloc(&ob.idx_in, sizeof(int32_t) * n)) == cudaSuccess &&
+        (err = cudaMalloc(&ob.idx_out, sizeof(int32_t) * n)) == cudaSuccess &&
+        (err = cub::DeviceRadixSort::SortPairsDescending(nullptr, ob.tmp_bytes, ob.key_in, ob.key_out, ob.idx_in,
+                                                         ob.idx_out, n, 0, 32, (cudaStream_t)0)) == cudaSuccess)
+        err = cudaMalloc(&ob.tmp, ob.tmp_bytes ? ob.tmp_bytes : 1);
+    if (err != cudaSuccess) adaptive_order_free(ob);
+    return err;
+}
+
 cudaError_t adaptive_order(const View& v, double t_end, OrderBuffers& ob, cudaStream_t s) {
+    if (!ob.key_in || !ob.key_out || !ob.idx_in || !ob.idx_out || !ob.tmp) return cudaErrorInvalidValue;
     cudaError_t err = cudaSuccess;
     const int n = (int)v.n_sys;
-    if (!ob.key_in) {
-        if ((err = cudaMalloc(&ob.key_in, sizeof(float) * n)) != cudaSuccess) return err;
-        if ((err = cudaMalloc(&ob.key_out, sizeof(float) * n)) != cudaSuccess) return err;
-        if ((err = cudaMalloc(&ob.idx_in, sizeof(int32_t) * n)) != cudaSuccess) return err;
-        if ((err = cudaMalloc(&ob.idx_out, sizeof(int32_t) * n)) != cudaSuccess) return err;
-        err = cub::DeviceRadixSort::SortPairsDescending(nullptr, ob.tmp_bytes, ob.key_in, ob.key_out, ob.idx_in,
-                                                        ob.idx_out, n, 0, 32, s);
-        if (err != cudaSuccess) return err;
-        if ((err = cudaMalloc(&ob.tmp, ob.tmp_bytes)) != cudaSuccess) return err;
-    }
     order_key_kernel<<<(unsigned)((v.n_sys + 127) / 128), 128, 0, s>>>(v, t_end, ob.key_in, ob.idx_in);
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     return cub::DeviceRadixSort::SortPairsDescending(ob.tmp, ob.tmp_bytes, ob.key_in, ob.key_out, ob.idx_in, ob.idx_out,

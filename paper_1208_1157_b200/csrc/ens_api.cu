@@ -4,7 +4,6 @@
 #include <cfloat>
 #include <cmath>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -316,28 +315,59 @@ __global__ void log_reset_kernel(int64_t* last, int64_t n, unsigned long long* c
 }  // namespace
 
 struct ens {
-    ensd::View v;
-    double r_close, r_eject;
-    bool have_state;
-    int device;
-    // device staging (AoS) for host-space calls, allocated on first use
-    double* stage;        // [n_sys * n_body * 7] : pos | vel | mass
-    double* stage_small;  // [n_sys * 4] : time / E | L   (also int32 status, int64 nsteps reuse)
-    ensd::KernelInfo hermite, hermite_adaptive, hermite_carry, rkck, mvs;
-    unsigned long long* counter;  // work counter of the adaptive kernels
-    ensd::OrderBuffers order;     // hand-out order of the adaptive kernels (allocated on first use)
-    int threads_override;
-    int64_t last_blocks;
-    const void* last_fn;
-    int64_t launches;
-    cudaEvent_t ev0, ev1;
-    bool timed;
-    LogView log;  // capacity 0 = no log buffer
+    ensd::View v{};
+    double r_close = 0.0, r_eject = INFINITY;
+    bool have_state = false;
+    int device = 0;
+    // device staging (AoS) for host-space calls, allocated by the first host-space call (which waits for the stream
+    // anyway) or ahead of time by ens_reserve_host_staging
+    // (a lazily filled cache: the read-only calls may fill it too, hence mutable)
+    mutable double* stage = nullptr;        // [n_sys * n_body * 7] : pos | vel | mass
+    mutable double* stage_small = nullptr;  // [n_sys * 4] : time / E | L
+    ensd::KernelInfo hermite{}, hermite_sliced{}, hermite_adaptive{}, hermite_carry{}, rkck{}, mvs{};
+    unsigned long long* counter = nullptr;  // work counter of the persistent kernels
+    int32_t* slice_done = nullptr;          // per warp-group slice counters of the time-sliced Hermite kernel
+    ensd::OrderBuffers order;               // hand-out order of the adaptive kernels (allocated by ens_create)
+    ensd::LaunchTune tune;                  // ens_test_set_option
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    LogView log{};  // capacity 0 = no log buffer
+    // bookkeeping that the read-only calls (ens_get_state, ens_energy) update too
+    mutable int64_t last_blocks = 0;
+    mutable const void* last_fn = nullptr;
+    mutable int64_t launches = 0;
+    mutable bool timed = false;
 };
 
 namespace {
 
-int ensure_stage(ens* e) {
+// Every entry point runs on the device the handle was created on, whatever device is current in the calling thread,
+// and leaves the caller's current device as it found it.
+class DeviceGuard {
+  public:
+    explicit DeviceGuard(int want) {
+        if (cudaGetDevice(&prev_) != cudaSuccess) { err_ = cudaGetLastError(); return; }
+        if (prev_ != want) {
+            err_ = cudaSetDevice(want);
+            switched_ = err_ == cudaSuccess;
+        }
+    }
+    ~DeviceGuard() {
+        if (switched_) cudaSetDevice(prev_);
+    }
+    cudaError_t error() const { return err_; }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+
+  private:
+    int prev_ = 0;
+    bool switched_ = false;
+    cudaError_t err_ = cudaSuccess;
+};
+#define ENS_ON_DEVICE(e)                 \
+    DeviceGuard guard__((e)->device);    \
+    CU(guard__.error())
+
+int ensure_stage(const ens* e) {
     const int64_t n = e->v.n_sys, nb = e->v.n_body;
     if (!e->stage) CU(cudaMalloc(&e->stage, sizeof(double) * n * nb * 7));
     if (!e->stage_small) CU(cudaMalloc(&e->stage_small, sizeof(double) * n * 4));
@@ -369,13 +399,10 @@ int ens_create(int64_t n_sys, int n_body, ens_t** out) {
     CU(cudaGetDevice(&dev));
     ens* e = new (std::nothrow) ens();
     if (!e) return ENS_ENOMEM;
-    memset(e, 0, sizeof *e);
     e->device = dev;
     e->v.n_sys = n_sys;
     e->v.n_body = n_body;
     e->v.n_pad = (n_sys + TILE - 1) / TILE * TILE;
-    e->r_close = 0.0;
-    e->r_eject = INFINITY;
     const int64_t np = e->v.n_pad;
     cudaError_t err = cudaSuccess;
     auto alloc = [&](void** p, size_t bytes) {
@@ -388,6 +415,9 @@ int ens_create(int64_t n_sys, int n_body, ens_t** out) {
     alloc((void**)&e->v.status, sizeof(int32_t) * np);
     alloc((void**)&e->v.nsteps, sizeof(int64_t) * np);
     alloc((void**)&e->counter, sizeof(unsigned long long));
+    alloc((void**)&e->slice_done, sizeof(int32_t) * (size_t)ensd::hermite_slice_groups(n_sys, n_body));
+    // everything ens_integrate needs is allocated here: device-space calls only enqueue
+    if (err == cudaSuccess && n_sys <= 0x7fffffff) err = ensd::adaptive_order_alloc(n_sys, e->order);
     if (err == cudaSuccess) err = cudaEventCreate(&e->ev0);
     if (err == cudaSuccess) err = cudaEventCreate(&e->ev1);
     if (err != cudaSuccess) {
@@ -398,41 +428,49 @@ int ens_create(int64_t n_sys, int n_body, ens_t** out) {
     e->hermite = ensd::hermite_kernel_for(n_body, 0);
     e->hermite_adaptive = ensd::hermite_kernel_for(n_body, 1);
     e->hermite_carry = ensd::hermite_kernel_for(n_body, 2);
+    e->hermite_sliced = ensd::hermite_kernel_for(n_body, 3);
     e->rkck = ensd::rkck_kernel_for(n_body);
     e->mvs = ensd::mvs_kernel_for(n_body);
-    const char* env = getenv("ENS_THREADS");
-    e->threads_override = env ? atoi(env) : 0;
-    if (e->threads_override < 32 || e->threads_override > 1024 || (e->threads_override & 31)) e->threads_override = 0;
     *out = e;
     return ENS_OK;
 }
 
 int ens_destroy(ens_t* e) {
     if (!e) return ENS_OK;
-    cudaDeviceSynchronize();
-    cudaFree(e->v.pos);
-    cudaFree(e->v.vel);
-    cudaFree(e->v.mass);
-    cudaFree(e->v.time);
-    cudaFree(e->v.status);
-    cudaFree(e->v.nsteps);
-    cudaFree(e->counter);
-    cudaFree(e->log.cursor);
-    cudaFree(e->log.last);
-    cudaFree(e->log.sys);
-    cudaFree(e->log.nsteps);
-    cudaFree(e->log.time);
-    cudaFree(e->log.status);
-    cudaFree(e->log.pos);
-    cudaFree(e->log.vel);
-    ensd::adaptive_order_free(e->order);
-    cudaFree(e->stage);
-    cudaFree(e->stage_small);
-    if (e->ev0) cudaEventDestroy(e->ev0);
-    if (e->ev1) cudaEventDestroy(e->ev1);
-    (void)cudaGetLastError();
+    {
+        DeviceGuard guard(e->device);
+        cudaDeviceSynchronize();
+        cudaFree(e->v.pos);
+        cudaFree(e->v.vel);
+        cudaFree(e->v.mass);
+        cudaFree(e->v.time);
+        cudaFree(e->v.status);
+        cudaFree(e->v.nsteps);
+        cudaFree(e->counter);
+        cudaFree(e->slice_done);
+        cudaFree(e->log.cursor);
+        cudaFree(e->log.last);
+        cudaFree(e->log.sys);
+        cudaFree(e->log.nsteps);
+        cudaFree(e->log.time);
+        cudaFree(e->log.status);
+        cudaFree(e->log.pos);
+        cudaFree(e->log.vel);
+        ensd::adaptive_order_free(e->order);
+        cudaFree(e->stage);
+        cudaFree(e->stage_small);
+        if (e->ev0) cudaEventDestroy(e->ev0);
+        if (e->ev1) cudaEventDestroy(e->ev1);
+        (void)cudaGetLastError();
+    }
     delete e;
     return ENS_OK;
+}
+
+int ens_reserve_host_staging(ens_t* e) {
+    if (!e) return ENS_EINVAL;
+    ENS_ON_DEVICE(e);
+    return ensure_stage(e);
 }
 
 int ens_set_monitors(ens_t* e, double r_close, double r_eject) {
@@ -445,6 +483,7 @@ int ens_set_monitors(ens_t* e, double r_close, double r_eject) {
 int ens_set_state(ens_t* e, const double* pos, const double* vel, const double* mass, const double* time, int memspace,
                   void* stream) {
     if (!e || !pos || !vel || !mass || (memspace != ENS_HOST && memspace != ENS_DEVICE)) return ENS_EINVAL;
+    ENS_ON_DEVICE(e);
     cudaStream_t s = (cudaStream_t)stream;
     const int64_t n = e->v.n_sys, nb = e->v.n_body;
     const double *dpos = pos, *dvel = vel, *dmass = mass, *dtime = time;
@@ -476,8 +515,9 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
     if (!e || integrator < ENS_HERMITE || integrator > ENS_RKCK) return ENS_EINVAL;
     if (!(dt != 0.0) || !std::isfinite(dt) || std::isnan(t_end) || max_steps < 0) return ENS_EINVAL;
     if (!e->have_state) return ENS_ESTATE;
+    ENS_ON_DEVICE(e);
     cudaStream_t s = (cudaStream_t)stream;
-    ensd::StepArgs a;
+    ensd::StepArgs a{};
     a.dt = dt;
     a.t_end = t_end;
     a.max_steps = max_steps;
@@ -489,9 +529,10 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
     ensd::fill_step_constants(a);
     a.counter = e->counter;
     a.order = nullptr;
+    a.slice_done = e->slice_done;
     if (integrator == ENS_HERMITE_ADAPTIVE) {
         CU(cudaMemsetAsync(e->counter, 0, sizeof(unsigned long long), s));
-        if (!getenv("ENS_ADAPTIVE_UNORDERED") && e->v.n_sys <= 0x7fffffff) {  // int32 indices in the sort  // (the switch exists for the measurement in DESIGN.md §8)
+        if (!e->tune.adaptive_unordered && e->order.idx_out) {
             CU(ensd::adaptive_order(e->v, t_end, e->order, s));
             a.order = e->order.idx_out;
             e->launches += 1;  // the key kernel (the sort is cub's)
@@ -503,17 +544,18 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
                                  : integrator == ENS_RKCK             ? e->rkck
                                                                       : e->mvs;
     if (!ki.fn) return ENS_EUNSUPPORTED;
-    const int threads = e->threads_override ? e->threads_override : ki.threads;
+    const int threads = e->tune.threads ? e->tune.threads : ki.threads;
+    const void* fn = ki.fn;
     CU(cudaEventRecord(e->ev0, s));
     cudaError_t err = integrator == ENS_MVS
                           ? ensd::launch_mvs(e->v, a, threads, s, &e->last_blocks)
                       : integrator == ENS_RKCK
                           ? ensd::launch_rkck(e->v, a, threads, s, &e->last_blocks)
                           : ensd::launch_hermite(e->v, a, integrator == ENS_HERMITE_ADAPTIVE ? 1 : integrator == ENS_HERMITE_CARRY ? 2 : 0,
-                                                 threads, s, &e->last_blocks);
+                                                 e->tune, s, &e->last_blocks, &fn);
     if (err != cudaSuccess) return cuda_fail(err, "ens_integrate launch");
     CU(cudaEventRecord(e->ev1, s));
-    e->last_fn = ki.fn;
+    e->last_fn = fn;
     e->launches += 1;
     e->timed = true;
     return ENS_OK;
@@ -523,12 +565,12 @@ int ens_get_state(const ens_t* e, double* pos, double* vel, double* time, int32_
                   int memspace, void* stream) {
     if (!e || (memspace != ENS_HOST && memspace != ENS_DEVICE)) return ENS_EINVAL;
     if (!e->have_state) return ENS_ESTATE;
-    ens* me = const_cast<ens*>(e);
+    ENS_ON_DEVICE(e);
     cudaStream_t s = (cudaStream_t)stream;
     const int64_t n = e->v.n_sys, nb = e->v.n_body;
     const cudaMemcpyKind kind = memspace == ENS_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
     if (memspace == ENS_HOST && (pos || vel)) {
-        const int rc = ensure_stage(me);
+        const int rc = ensure_stage(e);
         if (rc) return rc;
     }
     const bool dev = memspace == ENS_DEVICE;
@@ -536,7 +578,7 @@ int ens_get_state(const ens_t* e, double* pos, double* vel, double* time, int32_
         double* dp = !pos ? nullptr : dev ? pos : e->stage;
         double* dv = !vel ? nullptr : dev ? vel : e->stage + n * nb * 3;
         CU(launch_unpack(e->v, dp, dv, dev ? time : nullptr, dev ? status : nullptr, dev ? nsteps : nullptr, s));
-        me->launches += 1;
+        e->launches += 1;
         if (!dev) {
             if (pos) CU(cudaMemcpyAsync(pos, dp, sizeof(double) * n * nb * 3, kind, s));
             if (vel) CU(cudaMemcpyAsync(vel, dv, sizeof(double) * n * nb * 3, kind, s));
@@ -555,12 +597,12 @@ int ens_get_state(const ens_t* e, double* pos, double* vel, double* time, int32_
 int ens_energy(const ens_t* e, double* E, double* L, int memspace, void* stream) {
     if (!e || !E || (memspace != ENS_HOST && memspace != ENS_DEVICE)) return ENS_EINVAL;
     if (!e->have_state) return ENS_ESTATE;
-    ens* me = const_cast<ens*>(e);
+    ENS_ON_DEVICE(e);
     cudaStream_t s = (cudaStream_t)stream;
     const int64_t n = e->v.n_sys;
     double *dE = E, *dL = L;
     if (memspace == ENS_HOST) {
-        const int rc = ensure_stage(me);
+        const int rc = ensure_stage(e);
         if (rc) return rc;
         dE = e->stage_small;
         dL = L ? e->stage_small + n : nullptr;
@@ -571,7 +613,7 @@ int ens_energy(const ens_t* e, double* E, double* L, int memspace, void* stream)
         ENS_FOR_EACH_NB(X)
 #undef X
     }
-    me->launches += 1;
+    e->launches += 1;
     CU(cudaGetLastError());
     if (memspace == ENS_HOST) {
         CU(cudaMemcpyAsync(E, dE, sizeof(double) * n, cudaMemcpyDeviceToHost, s));
@@ -583,12 +625,13 @@ int ens_energy(const ens_t* e, double* E, double* L, int memspace, void* stream)
 
 int ens_log_enable(ens_t* e, int64_t capacity, void* stream) {
     if (!e || capacity < 0) return ENS_EINVAL;
+    ENS_ON_DEVICE(e);
     cudaStream_t s = (cudaStream_t)stream;
     CU(cudaStreamSynchronize(s));
     LogView& g = e->log;
     cudaFree(g.cursor); cudaFree(g.last); cudaFree(g.sys); cudaFree(g.nsteps);
     cudaFree(g.time); cudaFree(g.status); cudaFree(g.pos); cudaFree(g.vel);
-    memset(&g, 0, sizeof g);
+    g = LogView{};
     if (capacity == 0) return ENS_OK;
     const int64_t n3 = (int64_t)e->v.n_body * 3;
     CU(cudaMalloc(&g.cursor, sizeof(unsigned long long)));
@@ -610,6 +653,7 @@ int ens_integrate_logged(ens_t* e, int integrator, double dt, double t_end, int6
                          int what, void* stream) {
     if (!e || log_every < 1 || !(what & (ENS_LOG_SNAPSHOTS | ENS_LOG_STOPS))) return ENS_EINVAL;
     if (e->log.capacity == 0) return ENS_ESTATE;
+    ENS_ON_DEVICE(e);
     cudaStream_t s = (cudaStream_t)stream;
     int64_t done = 0;
     do {  // segments of log_every steps, each followed by the log kernel: all enqueued, no host round trip
@@ -628,6 +672,7 @@ int ens_log_read(const ens_t* e, int64_t* n_records, int64_t* n_dropped, int64_t
                  int32_t* status, double* pos, double* vel, int64_t max_records, int memspace, void* stream) {
     if (!e || !n_records || max_records < 0 || (memspace != ENS_HOST && memspace != ENS_DEVICE)) return ENS_EINVAL;
     if (e->log.capacity == 0) return ENS_ESTATE;
+    ENS_ON_DEVICE(e);
     cudaStream_t s = (cudaStream_t)stream;
     const LogView& g = e->log;
     unsigned long long cur = 0;
@@ -653,26 +698,26 @@ int ens_log_read(const ens_t* e, int64_t* n_records, int64_t* n_dropped, int64_t
 
 int ens_get_info(const ens_t* e, int64_t out[8]) {
     if (!e || !out) return ENS_EINVAL;
-    const ensd::KernelInfo& ki = (e->last_fn && e->last_fn == e->mvs.fn)                ? e->mvs
-                                 : (e->last_fn && e->last_fn == e->hermite_adaptive.fn) ? e->hermite_adaptive
-                                 : (e->last_fn && e->last_fn == e->hermite_carry.fn)    ? e->hermite_carry
-                                 : (e->last_fn && e->last_fn == e->rkck.fn)             ? e->rkck
-                                                                                        : e->hermite;
-    const int threads = e->threads_override ? e->threads_override : ki.threads;
+    ENS_ON_DEVICE(e);
+    const ensd::KernelInfo* all[] = {&e->mvs, &e->hermite_adaptive, &e->hermite_carry, &e->hermite_sliced, &e->rkck};
+    const ensd::KernelInfo* ki = &e->hermite;
+    for (const ensd::KernelInfo* c : all)
+        if (e->last_fn && e->last_fn == c->fn) ki = c;
+    const int threads = e->tune.threads ? e->tune.threads : ki->threads;
     out[0] = e->v.n_pad;
-    out[1] = ki.shape.L;
-    out[2] = ki.shape.B;
+    out[1] = ki->shape.L;
+    out[2] = ki->shape.B;
     out[3] = threads;
-    const int64_t sys_per_warp = 32 / (ki.shape.L > 0 ? ki.shape.L : 1);
+    const int64_t sys_per_warp = 32 / (ki->shape.L > 0 ? ki->shape.L : 1);
     const int64_t warps = (e->v.n_sys + sys_per_warp - 1) / sys_per_warp;
     out[4] = e->last_blocks ? e->last_blocks : (warps + threads / 32 - 1) / (threads / 32);
     out[5] = out[6] = 0;
-    if (ki.fn) {
+    if (ki->fn) {
         cudaFuncAttributes fa;
-        CU(cudaFuncGetAttributes(&fa, ki.fn));
+        CU(cudaFuncGetAttributes(&fa, ki->fn));
         out[5] = fa.numRegs;
         int nb = 0;
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, ki.fn, threads, 0));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, ki->fn, threads, 0));
         out[6] = nb;
     }
     out[7] = e->launches;
@@ -682,6 +727,7 @@ int ens_get_info(const ens_t* e, int64_t out[8]) {
 int ens_last_kernel_ms(const ens_t* e, float* ms) {
     if (!e || !ms) return ENS_EINVAL;
     if (!e->timed) return ENS_ESTATE;
+    ENS_ON_DEVICE(e);
     CU(cudaEventSynchronize(e->ev1));
     CU(cudaEventElapsedTime(ms, e->ev0, e->ev1));
     return ENS_OK;
@@ -693,25 +739,50 @@ int ens_fp64_peak(int64_t iters, double* lane_fma_per_s, void* stream) {
     int dev = 0, sms = 0;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    double* out = nullptr;
-    CU(cudaMalloc(&out, sizeof(double)));
-    cudaEvent_t a, b;
-    CU(cudaEventCreate(&a));
-    CU(cudaEventCreate(&b));
+    struct Scratch {  // released on every return path
+        double* out = nullptr;
+        cudaEvent_t a = nullptr, b = nullptr;
+        ~Scratch() {
+            if (a) cudaEventDestroy(a);
+            if (b) cudaEventDestroy(b);
+            cudaFree(out);
+        }
+    } w;
+    CU(cudaMalloc(&w.out, sizeof(double)));
+    CU(cudaEventCreate(&w.a));
+    CU(cudaEventCreate(&w.b));
     const int blocks = sms * 8, threads = 256;  // 64 warps per SM
-    dfma_kernel<<<blocks, threads, 0, s>>>(iters / 8 + 1, 1.0, out);  // warm-up
-    CU(cudaEventRecord(a, s));
-    dfma_kernel<<<blocks, threads, 0, s>>>(iters, 1.0, out);
-    CU(cudaEventRecord(b, s));
-    CU(cudaEventSynchronize(b));
+    dfma_kernel<<<blocks, threads, 0, s>>>(iters / 8 + 1, 1.0, w.out);  // warm-up
+    CU(cudaEventRecord(w.a, s));
+    dfma_kernel<<<blocks, threads, 0, s>>>(iters, 1.0, w.out);
+    CU(cudaEventRecord(w.b, s));
+    CU(cudaEventSynchronize(w.b));
     float ms = 0.f;
-    CU(cudaEventElapsedTime(&ms, a, b));
-    cudaEventDestroy(a);
-    cudaEventDestroy(b);
-    cudaFree(out);
+    CU(cudaEventElapsedTime(&ms, w.a, w.b));
     CU(cudaGetLastError());
     *lane_fma_per_s = (double)blocks * threads * (double)iters * 64.0 / (ms * 1e-3);
     return ENS_OK;
+}
+
+int ens_test_set_option(ens_t* e, int option, int64_t value) {
+    if (!e || value < 0) return ENS_EINVAL;
+    switch (option) {
+        case ENS_OPT_THREADS:
+            if (value != 0 && (value < 32 || value > 1024 || (value & 31))) return ENS_EINVAL;
+            e->tune.threads = (int)value;
+            return ENS_OK;
+        case ENS_OPT_ADAPTIVE_UNORDERED: e->tune.adaptive_unordered = value != 0; return ENS_OK;
+        case ENS_OPT_SLICE_MODE:
+            if (value > 2) return ENS_EINVAL;
+            e->tune.slice_mode = (int)value;
+            return ENS_OK;
+        case ENS_OPT_SLICE_STEPS: e->tune.slice_steps = value; return ENS_OK;
+        case ENS_OPT_SLICE_WARPS_PER_SM:
+            if (value > 64) return ENS_EINVAL;
+            e->tune.slice_warps_per_sm = (int)value;
+            return ENS_OK;
+    }
+    return ENS_EINVAL;
 }
 
 }  // extern "C"

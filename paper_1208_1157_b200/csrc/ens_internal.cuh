@@ -36,8 +36,12 @@ struct StepArgs {
     //   C_x = x + h v + cx_a a0 + cx_j j0            C_v = v + cv_a a0 + cv_j j0
     //   x_c = C_x + kx_a a1 + kx_j j1                v_c = C_v + kv_a a1 + kv_j j1
     double p_a, p_j, cx_a, cx_j, cv_a, cv_j, kx_a, kx_j, kv_a, kv_j;
-    unsigned long long* counter;  // adaptive kernels: next system index to hand out (zeroed before the launch)
+    unsigned long long* counter;  // persistent kernels: next system / task index to hand out (zeroed before the launch)
     const int32_t* order;         // adaptive kernels: hand-out order (longest expected run first), or nullptr
+    // time-sliced fixed-step kernel (hermite_kernel<..., SLICED>): tasks = (warp-group of systems, slice of slice_steps
+    // steps), handed out slice-major; slice_done[g] = slices group g has completed (zeroed before the launch)
+    int32_t* slice_done;
+    int64_t slice_steps, n_slices, n_groups;
 };
 
 inline void fill_step_constants(StepArgs& a) {
@@ -66,6 +70,15 @@ struct KernelInfo {
     int threads;  // threads per block
 };
 
+// Launch-time choices a test or a measurement may override through ens_test_set_option (0 = the library's default).
+struct LaunchTune {
+    int threads = 0;             // threads per block
+    int adaptive_unordered = 0;  // 1: hand the systems of the adaptive kernels out in index order
+    int slice_mode = 0;          // fixed-step Hermite: 0 = library decides, 1 = always time-sliced, 2 = never
+    int64_t slice_steps = 0;     // steps per slice
+    int slice_warps_per_sm = 0;  // persistent warps per SM of the time-sliced grid
+};
+
 // adaptive_order.cu: order[] = system indices sorted by decreasing expected number of adaptive steps
 struct OrderBuffers {
     float *key_in = nullptr, *key_out = nullptr;
@@ -73,13 +86,16 @@ struct OrderBuffers {
     void* tmp = nullptr;
     size_t tmp_bytes = 0;
 };
+cudaError_t adaptive_order_alloc(int64_t n_sys, OrderBuffers& ob);  // complete or empty
 cudaError_t adaptive_order(const View& v, double t_end, OrderBuffers& ob, cudaStream_t s);
 void adaptive_order_free(OrderBuffers& ob);
 
 // hermite_*.cu / mvs.cu
 KernelInfo hermite_kernel_for(int n_body, int mode);  // mode: 0 fixed step, 1 adaptive, 2 carried a/j
-cudaError_t launch_hermite(const View& v, const StepArgs& a, int mode, int threads, cudaStream_t s,
-                           int64_t* blocks_out);
+// slice_done: int32 [hermite_slice_groups(n_sys, n_body)] scratch of the time-sliced kernel (or nullptr: never sliced)
+int64_t hermite_slice_groups(int64_t n_sys, int n_body);
+cudaError_t launch_hermite(const View& v, const StepArgs& a, int mode, const LaunchTune& tune, cudaStream_t s,
+                           int64_t* blocks_out, const void** fn_out);
 KernelInfo rkck_kernel_for(int n_body);
 cudaError_t launch_rkck(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out);
 KernelInfo mvs_kernel_for(int n_body);

@@ -1,4 +1,6 @@
 // hermite.cu — instantiations of the fused Hermite step-loop kernel and the n_body -> (L, B) dispatch.
+#include <cmath>
+
 #include "hermite_kernel.cuh"
 
 namespace ensd {
@@ -6,77 +8,44 @@ namespace ensd {
 namespace {
 
 // n_body -> lanes per system L (odd), bodies per lane B, L * B >= n_body.  Exact fits for 2-6, 9, 10, 12, 15;
-// the others run in the next larger shape with massless dummy slots.
+// the others run in the next larger shape with massless dummy slots.  The values are the winners of the sweeps
+// recorded in DESIGN.md section 8 (tuning record).
+//   UNROLL   three inlined copies of the evaluation (straight-line step) instead of a 3-phase loop around one copy
+//   THREADS  threads per block;  MAXT, MINB = __launch_bounds__ (register cap 65536 / (MAXT * MINB))
 template <int N> struct ShapeOf;
-#define ENS_SHAPE(N_, L_, B_, UNROLL_, THREADS_, MINB_) ENS_SHAPE_T(N_, L_, B_, UNROLL_, THREADS_, MINB_, 128)
-#define ENS_SHAPE_T(N_, L_, B_, UNROLL_, THREADS_, MINB_, MAXT_)                        \
-    template <> struct ShapeOf<N_> {                                                    \
+#define ENS_SHAPE(N_, L_, B_, UNROLL_, THREADS_, MINB_, MAXT_)                              \
+    template <> struct ShapeOf<N_> {                                                        \
         static constexpr int L = L_, B = B_, THREADS = THREADS_, MINB = MINB_, MAXT = MAXT_; \
-        static constexpr bool UNROLL = UNROLL_;                                         \
+        static constexpr bool UNROLL = UNROLL_;                                             \
     };
-// Tuning knobs of the headline shape (n_body = 3), overridable at compile time for the sweeps recorded in DESIGN.md §8.
-#ifndef ENS_H3_UNROLL
-#define ENS_H3_UNROLL true
-#endif
-#ifndef ENS_H3_THREADS
-#define ENS_H3_THREADS 64
-#endif
-#ifndef ENS_H3_MAXT
-#define ENS_H3_MAXT 64  // __launch_bounds__ threads: with MINB it sets the register cap 65536 / (MAXT * MINB)
-#endif
-#ifndef ENS_H3_MINB
-#define ENS_H3_MINB 7  // register cap 128 (125 used, no spills), 8 blocks of 2 warps per SM (sweeps: DESIGN.md §8)
-#endif
-//        N  L  B  unroll threads minBlocks
-ENS_SHAPE(2, 1, 2, true, 64, 1)
-ENS_SHAPE_T(3, 1, 3, ENS_H3_UNROLL, ENS_H3_THREADS, ENS_H3_MINB, ENS_H3_MAXT)
-ENS_SHAPE(4, 1, 4, true, 64, 1)
-ENS_SHAPE(5, 1, 5, true, 64, 1)
+//        N  L  B  unroll threads minBlocks maxThreads
+ENS_SHAPE(2, 1, 2, true, 64, 1, 128)
+// n_body = 3 (config 1, the metric): register cap 128 (125 used, no spills), 8 blocks of 2 warps per SM
+ENS_SHAPE(3, 1, 3, true, 64, 7, 64)
+ENS_SHAPE(4, 1, 4, true, 64, 1, 128)
+ENS_SHAPE(5, 1, 5, true, 64, 1, 128)
 // n_body = 6 (config 2): one system per thread, all 15 pairs in one lane, no shuffles: 0.62 of FP64 issue peak against
-// 0.54 for the best 3-lane shape; 32-thread blocks spread the 1024 warps of config 2 evenly over the SMs.
-#ifndef ENS_H6_L
-#define ENS_H6_L 1
-#define ENS_H6_B 6
-#endif
-#ifndef ENS_H6_THREADS
-#define ENS_H6_THREADS 32
-#define ENS_H6_MAXT 32
-#define ENS_H6_MINB 1
-#endif
-#ifndef ENS_H6_UNROLL
-#define ENS_H6_UNROLL true  // straight-line step (three copies of the 15-pair evaluation): 0.668 against 0.653 for the 3-phase loop
-#endif
-ENS_SHAPE_T(6, ENS_H6_L, ENS_H6_B, ENS_H6_UNROLL, ENS_H6_THREADS, ENS_H6_MINB, ENS_H6_MAXT)
-ENS_SHAPE(7, 3, 3, false, 64, 1)
-ENS_SHAPE(8, 3, 3, false, 64, 1)
-ENS_SHAPE(9, 3, 3, false, 64, 1)
-ENS_SHAPE(10, 5, 2, false, 64, 1)
-ENS_SHAPE(11, 3, 4, false, 64, 1)
-ENS_SHAPE(12, 3, 4, false, 64, 1)
-ENS_SHAPE(13, 5, 3, false, 64, 1)
-ENS_SHAPE(14, 5, 3, false, 64, 1)
-#ifndef ENS_H15_L
-#define ENS_H15_L 5
-#define ENS_H15_B 3
-#endif
-#ifndef ENS_H15_THREADS
-#define ENS_H15_THREADS 64
-#define ENS_H15_MAXT 128
-#define ENS_H15_MINB 1
-#endif
-#ifndef ENS_H15_UNROLL
-#define ENS_H15_UNROLL false
-#endif
-ENS_SHAPE_T(15, ENS_H15_L, ENS_H15_B, ENS_H15_UNROLL, ENS_H15_THREADS, ENS_H15_MINB, ENS_H15_MAXT)
-ENS_SHAPE(16, 5, 4, false, 64, 1)
+// 0.54 for the best 3-lane shape; 32-thread blocks spread the 1024 warps of config 2 evenly over the SMs; straight-line
+// step 0.668 against 0.653 for the 3-phase loop
+ENS_SHAPE(6, 1, 6, true, 32, 1, 32)
+ENS_SHAPE(7, 3, 3, false, 64, 1, 128)
+ENS_SHAPE(8, 3, 3, false, 64, 1, 128)
+ENS_SHAPE(9, 3, 3, false, 64, 1, 128)
+ENS_SHAPE(10, 5, 2, false, 64, 1, 128)
+ENS_SHAPE(11, 3, 4, false, 64, 1, 128)
+ENS_SHAPE(12, 3, 4, false, 64, 1, 128)
+ENS_SHAPE(13, 5, 3, false, 64, 1, 128)
+ENS_SHAPE(14, 5, 3, false, 64, 1, 128)
+ENS_SHAPE(15, 5, 3, false, 64, 1, 128)
+ENS_SHAPE(16, 5, 4, false, 64, 1, 128)
 #undef ENS_SHAPE
-#undef ENS_SHAPE_T
 
-// MODE: 0 = fixed step (3 evaluations), 1 = adaptive step, 2 = fixed step with carried a, j (2 evaluations)
+// MODE: 0 = fixed step (3 evaluations), 1 = adaptive step, 2 = fixed step with carried a, j (2 evaluations),
+//       3 = MODE 0 on a time-sliced persistent grid (same arithmetic, bit-identical results)
 template <int N, int MODE>
 constexpr auto kernel_ptr() {
     using S = ShapeOf<N>;
-    return &hermite_kernel<N, S::L, S::B, S::UNROLL, S::MAXT, S::MINB, MODE == 1, MODE == 2>;
+    return &hermite_kernel<N, S::L, S::B, S::UNROLL, S::MAXT, S::MINB, MODE == 1, MODE == 2, MODE == 3>;
 }
 
 template <int N, int MODE>
@@ -90,25 +59,69 @@ KernelInfo info_of() {
     return k;
 }
 
+// blocks of `threads` threads the device holds at once
 template <int N, int MODE>
-cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
+cudaError_t resident_blocks(int threads, int64_t* out) {
+    int dev = 0, sms = 0, per_sm = 0;
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel_ptr<N, MODE>(), threads, 0);
+    *out = (int64_t)sms * (per_sm > 0 ? per_sm : 1);
+    return err;
+}
+
+template <int N, int MODE>
+cudaError_t launch_n(const View& v, StepArgs a, const LaunchTune& tune, cudaStream_t s, int64_t* blocks_out,
+                     const void** fn_out) {
     using S = ShapeOf<N>;
+    int threads = tune.threads ? tune.threads : S::THREADS;
     if (threads > S::MAXT) threads = S::MAXT;  // __launch_bounds__ of the kernel
     const int64_t sys_per_warp = 32 / S::L;
     const int64_t warps = (v.n_sys + sys_per_warp - 1) / sys_per_warp;
     const int wpb = threads / 32;
     int64_t blocks = (warps + wpb - 1) / wpb;
+    cudaError_t err = cudaSuccess;
     if constexpr (MODE == 1) {  // persistent grid: what the device holds at once; lane groups pull systems from a.counter
-        int dev = 0, sms = 0, per_sm = 0;
-        cudaError_t err = cudaGetDevice(&dev);
-        if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (err == cudaSuccess)
-            err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel_ptr<N, MODE>(), threads, 0);
-        if (err != cudaSuccess) return err;
-        const int64_t resident = (int64_t)sms * (per_sm > 0 ? per_sm : 1);
+        int64_t resident = 0;
+        if ((err = resident_blocks<N, MODE>(threads, &resident)) != cudaSuccess) return err;
         if (blocks > resident) blocks = resident;
     }
+    if constexpr (MODE == 0) {
+        // Time slicing pays when the ensemble is more than one wave of resident warps but only a few: the last,
+        // partly filled wave would otherwise run a whole pass on a mostly empty device.
+        int64_t resident = 0;
+        if ((err = resident_blocks<N, 3>(threads, &resident)) != cudaSuccess) return err;
+        if (tune.slice_warps_per_sm > 0) {
+            int dev = 0, sms = 0;
+            if ((err = cudaGetDevice(&dev)) != cudaSuccess) return err;
+            if ((err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return err;
+            const int64_t want = ((int64_t)sms * tune.slice_warps_per_sm + wpb - 1) / wpb;
+            if (want < resident) resident = want;
+        }
+        const bool tail = blocks > resident && blocks < 4 * resident;
+        const bool sliced = a.slice_done && a.max_steps > 0 &&
+                            (tune.slice_mode == 1 || (tune.slice_mode == 0 && tail && a.max_steps >= 256));
+        if (sliced) {
+            // ~128 slices of the expected run (at least 32 steps each: a slice costs one extra evaluation + load/store)
+            double expect = (double)a.max_steps;
+            if (std::isfinite(a.t_end)) expect = fmin(expect, ceil(fabs(a.t_end / a.dt)) + 1.0);
+            int64_t k = tune.slice_steps > 0 ? tune.slice_steps : (int64_t)ceil(expect / 128.0);
+            if (tune.slice_steps <= 0 && k < 32) k = 32;
+            if (k > a.max_steps) k = a.max_steps;
+            a.slice_steps = k;
+            a.n_slices = (a.max_steps + k - 1) / k;
+            a.n_groups = warps;
+            if (blocks > resident) blocks = resident;
+            if ((err = cudaMemsetAsync(a.counter, 0, sizeof(unsigned long long), s)) != cudaSuccess) return err;
+            if ((err = cudaMemsetAsync(a.slice_done, 0, sizeof(int32_t) * (size_t)warps, s)) != cudaSuccess) return err;
+            if (blocks_out) *blocks_out = blocks;
+            if (fn_out) *fn_out = (const void*)kernel_ptr<N, 3>();
+            kernel_ptr<N, 3>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
+            return cudaGetLastError();
+        }
+    }
     if (blocks_out) *blocks_out = blocks;
+    if (fn_out) *fn_out = (const void*)kernel_ptr<N, MODE>();
     kernel_ptr<N, MODE>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
     return cudaGetLastError();
 }
@@ -120,7 +133,7 @@ cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t
 KernelInfo hermite_kernel_for(int n_body, int mode) {
     switch (n_body) {
 #define X(N_) \
-    case N_: return mode == 1 ? info_of<N_, 1>() : mode == 2 ? info_of<N_, 2>() : info_of<N_, 0>();
+    case N_: return mode == 1 ? info_of<N_, 1>() : mode == 2 ? info_of<N_, 2>() : mode == 3 ? info_of<N_, 3>() : info_of<N_, 0>();
         ENS_FOR_EACH_N(X)
 #undef X
     }
@@ -131,18 +144,28 @@ KernelInfo hermite_kernel_for(int n_body, int mode) {
     return none;
 }
 
-cudaError_t launch_hermite(const View& v, const StepArgs& a, int mode, int threads, cudaStream_t s,
-                           int64_t* blocks_out) {
+cudaError_t launch_hermite(const View& v, const StepArgs& a, int mode, const LaunchTune& tune, cudaStream_t s,
+                           int64_t* blocks_out, const void** fn_out) {
     switch (v.n_body) {
 #define X(N_) \
     case N_:  \
-        return mode == 1   ? launch_n<N_, 1>(v, a, threads, s, blocks_out) \
-               : mode == 2 ? launch_n<N_, 2>(v, a, threads, s, blocks_out) \
-                           : launch_n<N_, 0>(v, a, threads, s, blocks_out);
+        return mode == 1   ? launch_n<N_, 1>(v, a, tune, s, blocks_out, fn_out) \
+               : mode == 2 ? launch_n<N_, 2>(v, a, tune, s, blocks_out, fn_out) \
+                           : launch_n<N_, 0>(v, a, tune, s, blocks_out, fn_out);
         ENS_FOR_EACH_N(X)
 #undef X
     }
     return cudaErrorInvalidValue;
+}
+
+int64_t hermite_slice_groups(int64_t n_sys, int n_body) {
+    switch (n_body) {
+#define X(N_) \
+    case N_: return (n_sys + 32 / ShapeOf<N_>::L - 1) / (32 / ShapeOf<N_>::L);
+        ENS_FOR_EACH_N(X)
+#undef X
+    }
+    return 0;
 }
 
 namespace {

@@ -250,9 +250,17 @@ __device__ __forceinline__ int monitor_flags(const double (&x)[B][3], u64 r2min,
 // CARRY = true: Alg. 2 exactly as printed (reading R6-alt): two evaluations per step; (a0, j0) of a step
 // are the (a2, j2) the previous step's last evaluation left in the registers; only the first step of a launch
 // evaluates at the state itself.  A third less pair work per step; the step is no longer a pure function of (x, v).
-template <int N, int L, int B, bool UNROLL, int MAXT, int MINB, bool ADAPT = false, bool CARRY = false>
+// SLICED = true (fixed step, 3 evaluations): a persistent grid that time-slices the ensemble.  The step is a pure
+// function of the state (R6), so a run of max_steps steps equals ceil(max_steps / K) back-to-back runs of K steps with
+// the state parked in the SoA rows (L2-resident) in between, bit for bit.  Warps pull tasks (warp-group g of S systems,
+// slice s) from a device counter, slice-major, so all groups advance at the same rate and an ensemble of, say, 1.15
+// waves of resident warps keeps every warp slot busy until the last slice instead of running a second, nearly empty
+// wave for a whole pass (config 3: DESIGN.md section 6.1).  slice_done[g] orders slice s + 1 of a group after slice s.
+template <int N, int L, int B, bool UNROLL, int MAXT, int MINB, bool ADAPT = false, bool CARRY = false,
+          bool SLICED = false>
 __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p) {
     static_assert(!(ADAPT && CARRY), "the carried (a, j) are not kept across refills");
+    static_assert(!(SLICED && (ADAPT || CARRY)), "time slices need a step that is a pure function of the state");
     constexpr int S = 32 / L;  // systems per warp
     constexpr bool PADDED = (L * B != N);
     const int lane = threadIdx.x & 31;
@@ -270,7 +278,13 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
     int st = ENS_STOP_NONFINITE;
     bool active = false, writeback = false;
     int64_t k = 0;
+    int64_t kmax = p.max_steps;  // step budget of this run (SLICED: of the current slice)
 
+    // SLICED: another SM wrote these rows in the previous slice; read them from L2, never from a stale L1 line
+    auto ld = [](const auto* q) {
+        if constexpr (SLICED) return __ldcg(q);
+        else return *q;
+    };
     auto load_system = [&]() {  // sys -> registers; sets active / writeback
 #pragma unroll
         for (int b = 0; b < B; ++b) {
@@ -283,14 +297,14 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
             if (!PADDED || gid < N) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    X[b][c] = e.pos[(int64_t)(gid * 3 + c) * e.n_pad + sys];
-                    V[b][c] = e.vel[(int64_t)(gid * 3 + c) * e.n_pad + sys];
+                    X[b][c] = ld(&e.pos[(int64_t)(gid * 3 + c) * e.n_pad + sys]);
+                    V[b][c] = ld(&e.vel[(int64_t)(gid * 3 + c) * e.n_pad + sys]);
                 }
                 m[b] = e.mass[(int64_t)gid * e.n_pad + sys];
             }
         }
-        t = e.time[sys];
-        st = e.status[sys];
+        t = ld(&e.time[sys]);
+        st = ld(&e.status[sys]);
         k = 0;
         active = st < ENS_STOP_CLOSE;  // STOP_* are sticky; DONE_* run again
         writeback = active;
@@ -311,14 +325,14 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
             if (l == 0) {
                 e.time[sys] = t;
                 e.status[sys] = st;
-                e.nsteps[sys] += k;
+                e.nsteps[sys] = ld(&e.nsteps[sys]) + k;
             }
         }
         writeback = false;
     };
 
     bool exhausted = !(sl < S);  // ADAPT: this lane group will pull no more systems
-    if constexpr (!ADAPT) {
+    if constexpr (!ADAPT && !SLICED) {
 #pragma unroll
         for (int b = 0; b < B; ++b) {
             X[b][0] = 1.0e8 * (double)(l * B + b + 1);
@@ -374,7 +388,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
             if (!(fwd ? (t < p.t_end) : (t > p.t_end))) {
                 st = ENS_DONE_TIME;
                 active = false;
-            } else if (k >= p.max_steps) {
+            } else if (k >= kmax) {
                 st = ENS_DONE_STEPS;
                 active = false;
             }
@@ -425,6 +439,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
     };
 
     bool fresh = true;  // CARRY: a, j do not yet belong to the current state (warp-uniform: start of the launch)
+    auto run = [&]() {
     if constexpr (UNROLL) {
         while (true) {
             if constexpr (ADAPT) {
@@ -488,7 +503,52 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
             fresh = false;
         }
     }
-    store_system();
+    };
+    if constexpr (SLICED) {
+        const unsigned long long G = (unsigned long long)p.n_groups, n_tasks = G * (unsigned long long)p.n_slices;
+        while (true) {
+            unsigned long long task = 0;
+            if (lane == 0) task = atomicAdd(p.counter, 1ull);
+            task = __shfl_sync(0xffffffffu, task, 0);
+            if (task >= n_tasks) break;
+            const int64_t s = (int64_t)(task / G), g = (int64_t)(task - (unsigned long long)s * G);
+            if (s > 0) {  // slice s - 1 of this group is held by a running warp (tasks are handed out in order)
+                if (lane == 0) {
+                    int seen;
+                    while (true) {
+                        asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(p.slice_done + g) : "memory");
+                        if (seen >= (int)s) break;
+                        __nanosleep(200);
+                    }
+                }
+                __syncwarp();
+            }
+            sys = g * S + sl;
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                X[b][0] = 1.0e8 * (double)(l * B + b + 1);
+                X[b][1] = X[b][2] = 0.0;
+                V[b][0] = V[b][1] = V[b][2] = 0.0;
+                m[b] = 0.0;
+            }
+            active = writeback = false;
+            if ((sl < S) && (sys < e.n_sys)) {
+                load_system();
+                // a system that ran out of time in an earlier slice of this call is still out of time
+                if (s > 0 && st == ENS_DONE_TIME) active = writeback = false;
+            }
+            const int64_t left = p.max_steps - s * p.slice_steps;
+            kmax = left < p.slice_steps ? left : p.slice_steps;
+            run();
+            store_system();
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p.slice_done + g), "r"((int)s + 1) : "memory");
+        }
+    } else {
+        run();
+        store_system();
+    }
 }
 
 }  // namespace ensd

@@ -56,10 +56,13 @@ struct Stumpff {
 // period come here.
 __device__ __noinline__ Stumpff stumpff_general(double z) {
     int nq = 0;
-    while (fabs(z) > 0.1) {
+    // at most 540 quarterings bring any finite double below 0.1; +-inf and NaN leave the loop at the bound and give
+    // non-finite G functions, which the non-finite monitor reports (no endless loop on a broken state)
+    while (fabs(z) > 0.1 && nq < 540) {
         z *= 0.25;
         ++nq;
     }
+    if (!(fabs(z) <= 0.1)) z = __longlong_as_double(0x7ff8000000000000ll);
     Stumpff c;
     stumpff_series(z, c.c0, c.c1, c.c2, c.c3);
     for (; nq > 0; --nq) {

@@ -17,6 +17,7 @@ HERMITE, MVS, HERMITE_ADAPTIVE, HERMITE_CARRY, RKCK = 0, 1, 2, 3, 4  # HERMITE_A
 HOST, DEVICE = 0, 1
 ACTIVE, DONE_TIME, DONE_STEPS, STOP_CLOSE, STOP_EJECT, STOP_NONFINITE = range(6)
 LOG_SNAPSHOTS, LOG_STOPS = 1, 2
+OPT_THREADS, OPT_ADAPTIVE_UNORDERED, OPT_SLICE_MODE, OPT_SLICE_STEPS, OPT_SLICE_WARPS_PER_SM = range(5)
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libens.so")
@@ -24,7 +25,8 @@ LIB_PATH = os.path.join(_HERE, "libens.so")
 SYMBOLS = (
     "ens_create", "ens_destroy", "ens_set_state", "ens_set_monitors", "ens_integrate", "ens_get_state",
     "ens_energy", "ens_strerror", "ens_get_info", "ens_last_kernel_ms", "ens_fp64_peak", "ens_test_rsqrt",
-    "ens_test_rcp", "ens_log_enable", "ens_integrate_logged", "ens_log_read",
+    "ens_test_rcp", "ens_log_enable", "ens_integrate_logged", "ens_log_read", "ens_reserve_host_staging",
+    "ens_test_set_option",
 )
 _lib = None
 
@@ -69,6 +71,8 @@ def lib() -> ctypes.CDLL:
         L.ens_test_rcp.argtypes = [vp, vp, i64, vp]
         L.ens_log_enable.argtypes = [vp, i64, vp]
         L.ens_integrate_logged.argtypes = [vp, ci, cd, cd, i64, i64, ci, vp]
+        L.ens_reserve_host_staging.argtypes = [vp]
+        L.ens_test_set_option.argtypes = [vp, ci, i64]
         L.ens_log_read.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64), vp, vp, vp, vp, vp, vp, i64, ci, vp]
         for name in SYMBOLS:
             if name != "ens_strerror":
@@ -222,6 +226,12 @@ class Ensemble:
         return out
 
     # -- helpers ------------------------------------------------------------------------------------
+    def reserve_host_staging(self):
+        _check(lib().ens_reserve_host_staging(self._h), "ens_reserve_host_staging")
+
+    def set_option(self, option: int, value: int):
+        _check(lib().ens_test_set_option(self._h, int(option), int(value)), "ens_test_set_option")
+
     def info(self) -> dict:
         buf = (ctypes.c_int64 * 8)()
         _check(lib().ens_get_info(self._h, buf), "ens_get_info")

@@ -108,7 +108,7 @@ def test_monitors_split_runs_and_direction():
         assert (c["status"] == ens.DONE_TIME).all() and (c["time"] <= 0.0).all() and (c["time"] > -0.1).all()
 
 
-def test_results_do_not_depend_on_the_hand_out_order_and_stops_are_sticky(monkeypatch):
+def test_results_do_not_depend_on_the_hand_out_order_and_stops_are_sticky():
     """The longest-first hand-out (adaptive_order.cu) only schedules: with it switched off every system ends in the
     bit-identical state.  A system stopped by a monitor is not touched by a second call (it is pulled, found stopped,
     and retired without a write-back)."""
@@ -117,9 +117,8 @@ def test_results_do_not_depend_on_the_hand_out_order_and_stops_are_sticky(monkey
     vel[11, 2] = vel[11, 1] + np.array([-0.5, 0.0, 0.0])
     runs = []
     for unordered in (False, True):
-        if unordered:
-            monkeypatch.setenv("ENS_ADAPTIVE_UNORDERED", "1")
         with ens.Ensemble(3000, 3) as e:
+            e.set_option(ens.OPT_ADAPTIVE_UNORDERED, int(unordered))
             e.set_state(pos, vel, mass)
             e.set_monitors(0.02, 100.0)
             e.integrate(ens.HERMITE_ADAPTIVE, 0.03, 10**6, 6.0)

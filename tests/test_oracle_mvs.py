@@ -95,6 +95,90 @@ def test_kepler_drift_hyperbolic_conserves_orbit_invariants():
     assert np.abs(qc - q0).max() < 1e-13 and np.abs(pc - p0).max() < 1e-13
 
 
+# --------------------------------------------------------------------------- the bracket-and-bisect fallback (R-M4)
+# Newton's iteration of the oracle stops only at |dX| <= 1e-15 |X|; for steps of many radians of orbital phase the
+# correction ends up hovering at the rounding level (or the first guess X = tau / r0 is far off) and the 50-iteration
+# cap hands over to the monotone bracket-and-bisect branch.  These cases REACH that branch (asserted) and pin its
+# result to something that does not come from it.
+FALLBACK_ELLIPTIC = [  # (a, e, M0, tau): found by scanning, each takes the fallback in double precision
+    (1.0, 0.3, 0.7, 3.0), (1.0, 0.3, 2.0, -11.0), (1.0, 0.3, 5.5, -11.0), (1.0, 0.85, 0.7, 7.0), (1.0, 0.85, 5.5, 40.0),
+    (1.3, 0.3, 0.1, 7.0), (1.3, 0.3, 4.0, 40.0), (1.3, 0.6, 0.1, 40.0), (1.3, 0.85, 5.5, -11.0), (1.0, 0.0, 2.0, 100.0),
+    (1.0, 0.6, 4.0, 100.0), (0.4, 0.85, 5.5, 100.0), (1.3, 0.6, 2.0, 100.0),
+]
+
+
+@pytest.mark.parametrize("a,e,M0,tau", FALLBACK_ELLIPTIC)
+def test_kepler_drift_bisection_fallback_matches_keplers_equation(a, e, M0, tau):
+    """Multi-revolution and large-step elliptic drifts through the fallback against Kepler's equation solved
+    independently (workloads.elements_to_cartesian at the advanced mean anomaly)."""
+    mu = 1.0
+    q0, p0 = _kepler_state(a, e, M0, mu)
+    q1, p1, it = oracle.kepler_drift(q0, p0, mu, tau)
+    assert it < 0, "this case no longer reaches the fallback: replace it"
+    n = math.sqrt(mu / a**3)
+    qe, pe = _kepler_state(a, e, M0 + n * tau, mu)
+    tol = 3e-14 * (1 + n * abs(tau)) / (1 - e)  # rounding of the phase n tau, amplified near pericentre
+    np.testing.assert_allclose(q1, qe, rtol=0, atol=tol)
+    np.testing.assert_allclose(p1, pe, rtol=0, atol=tol / (1 - e))
+    # the same flow in extended precision (its own Newton run converges or falls back independently)
+    q2, p2, _ = oracle.kepler_drift(q0, p0, mu, tau, prec=oracle.LONG_DOUBLE)
+    np.testing.assert_allclose(q1, q2, rtol=0, atol=tol)
+
+
+def _hyperbolic_fallback_cases(n_want=8):
+    """Seeded unbound orbits (v^2 > 2 mu / r) with large steps that take the fallback in double precision."""
+    rng = np.random.default_rng(1)
+    cases = []
+    while len(cases) < n_want:
+        q0, p0 = rng.normal(size=3), rng.normal(size=3) * 1.5
+        tau = float(rng.choice([3.0, -11.0, 40.0]))
+        if p0 @ p0 <= 2.2 / np.linalg.norm(q0):
+            continue
+        if oracle.kepler_drift(q0, p0, 1.0, tau)[2] < 0:
+            cases.append((q0, p0, tau))
+    return cases
+
+
+@pytest.mark.parametrize("case", range(8))
+def test_kepler_drift_bisection_fallback_hyperbolic_invariants_and_group_property(case):
+    """Hyperbolic drifts through the fallback: energy, angular momentum and eccentricity vector are those of the start,
+    the time of flight from the hyperbolic Kepler equation M_h = e sinh H - H equals tau, and drift(tau) equals
+    drift(tau - s) after drift(s) for a small s that Newton handles (a result the fallback did not produce)."""
+    mu = 1.0
+    q0, p0, tau = _hyperbolic_fallback_cases()[case]
+    assert p0 @ p0 > 2 * mu / np.linalg.norm(q0)
+    q1, p1, it = oracle.kepler_drift(q0, p0, mu, tau)
+    assert it < 0
+
+    def invariants(q, p):
+        r = np.linalg.norm(q)
+        h = np.cross(q, p)
+        return p @ p / 2 - mu / r, h, np.cross(p, h) / mu - q / r
+
+    E0, h0, e0 = invariants(q0, p0)
+    E1, h1, e1 = invariants(q1, p1)
+    scale = 1 + abs(tau)
+    assert abs(E1 - E0) < 1e-14 * scale * abs(E0) and np.abs(h1 - h0).max() < 1e-14 * scale * np.linalg.norm(h0)
+    assert np.abs(e1 - e0).max() < 1e-14 * scale * np.linalg.norm(e0)
+
+    def mean_anomaly(q, p):  # hyperbolic: r = a (e cosh H - 1), q.p = sqrt(mu a) e sinh H, with a = mu / (2 E) > 0
+        a = mu / (2 * E0)
+        ecc = np.linalg.norm(e0)
+        sinhH = (q @ p) / (math.sqrt(mu * a) * ecc)
+        H = math.asinh(sinhH)
+        return ecc * sinhH - H, math.sqrt(mu / a**3)
+
+    M0, nh = mean_anomaly(q0, p0)
+    M1, _ = mean_anomaly(q1, p1)
+    assert abs((M1 - M0) / nh - tau) < 1e-13 * scale * max(1.0, abs(M1), abs(M0))
+    s = 0.01 * np.sign(tau)
+    qa, pa, ita = oracle.kepler_drift(q0, p0, mu, s)
+    assert ita > 0
+    qb, pb, _ = oracle.kepler_drift(qa, pa, mu, tau - s)
+    assert np.abs(qb - q1).max() < 1e-13 * scale * np.linalg.norm(q1)
+    assert np.abs(pb - p1).max() < 1e-13 * scale * np.linalg.norm(p1)
+
+
 def test_kepler_drift_long_double_agrees():
     q0, p0 = _kepler_state(0.7, 0.3, 2.0, 1.0)
     q1, p1, _ = oracle.kepler_drift(q0, p0, 1.0, 0.05)
