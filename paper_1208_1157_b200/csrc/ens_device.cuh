@@ -58,4 +58,11 @@ __device__ __forceinline__ void min_bits(u64& acc, double r2, bool valid = true)
     acc = b < acc ? b : acc;
 }
 
+// The same minimum on the high words only (exponent and top 20 mantissa bits): one integer min per value.  Exact
+// whenever the compared high words differ; the caller resolves ties (hermite_kernel.cuh: monitor_flags).
+__device__ __forceinline__ void min_hi(unsigned& acc, double r2, bool valid = true) {
+    const unsigned h = valid ? (unsigned)__double2hiint(r2) : ~0u;
+    acc = min(acc, h);
+}
+
 }  // namespace ensd

@@ -87,8 +87,10 @@ cudaError_t launch_n(const View& v, StepArgs a, const LaunchTune& tune, cudaStre
         if (blocks > resident) blocks = resident;
     }
     if constexpr (MODE == 0) {
-        // Time slicing pays when the ensemble is more than one wave of resident warps but only a few: the last,
-        // partly filled wave would otherwise run a whole pass on a mostly empty device.
+        // Time slicing pays when the ensemble is a few waves of resident warps and the last one is mostly empty: that
+        // wave would otherwise run a whole pass on a nearly idle device (config 3: 1.15 waves).  Measured (DESIGN.md
+        // section 8): a gain for the many-lane shapes (large state per warp, 2 warps per SM sub-partition); a loss
+        // for one-system-per-thread shapes, whose partly filled last wave still saturates the FP64 pipe.
         int64_t resident = 0;
         if ((err = resident_blocks<N, 3>(threads, &resident)) != cudaSuccess) return err;
         if (tune.slice_warps_per_sm > 0) {
@@ -98,14 +100,14 @@ cudaError_t launch_n(const View& v, StepArgs a, const LaunchTune& tune, cudaStre
             const int64_t want = ((int64_t)sms * tune.slice_warps_per_sm + wpb - 1) / wpb;
             if (want < resident) resident = want;
         }
-        const bool tail = blocks > resident && blocks < 4 * resident;
+        const bool tail = S::L > 1 && blocks > resident && blocks < 4 * resident && 2 * (blocks % resident) < resident;
         const bool sliced = a.slice_done && a.max_steps > 0 &&
                             (tune.slice_mode == 1 || (tune.slice_mode == 0 && tail && a.max_steps >= 256));
         if (sliced) {
-            // ~128 slices of the expected run (at least 32 steps each: a slice costs one extra evaluation + load/store)
+            // ~64 slices of the expected run (at least 32 steps each: a slice costs one extra evaluation + load/store)
             double expect = (double)a.max_steps;
             if (std::isfinite(a.t_end)) expect = fmin(expect, ceil(fabs(a.t_end / a.dt)) + 1.0);
-            int64_t k = tune.slice_steps > 0 ? tune.slice_steps : (int64_t)ceil(expect / 128.0);
+            int64_t k = tune.slice_steps > 0 ? tune.slice_steps : (int64_t)ceil(expect / 64.0);
             if (tune.slice_steps <= 0 && k < 32) k = 32;
             if (k > a.max_steps) k = a.max_steps;
             a.slice_steps = k;

@@ -57,101 +57,100 @@ __device__ __forceinline__ double pair_acc_jerk(const double (&xi)[3], const dou
 
 // Acceleration and jerk of the B bodies this lane owns, every pair of the system once.
 // l = lane index inside the system (0..L-1), base = first lane of the system in the warp, amask = active lanes.
-// TRACK = false skips the minimum pair distance (only a step's first evaluation feeds the monitor).
+// TRACK = false skips the minimum pair distance (only a step's first evaluation feeds the monitor).  The minimum is
+// kept as the smallest HIGH WORD of the squared separations' bit patterns (one integer min per pair, off the FP64
+// pipe); monitor_flags decides exactly from it, recomputing the full 64-bit minimum only in the rare tie.
 template <int N, int L, int B, bool TRACK = true>
 __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const double (&v)[B][3], const double (&m)[B],
-                                              double (&a)[B][3], double (&j)[B][3], u64& r2min, int l, int base,
+                                              double (&a)[B][3], double (&j)[B][3], unsigned& r2min, int l, int base,
                                               unsigned amask) {
     constexpr bool PADDED = (L * B != N);
 #pragma unroll
     for (int b = 0; b < B; ++b)
 #pragma unroll
         for (int c = 0; c < 3; ++c) a[b][c] = j[b][c] = 0.0;
-    if constexpr (TRACK) r2min = ~0ull;
+    if constexpr (TRACK) r2min = ~0u;
 
     // Cross-lane schedule (L > 1), written so that shuffle latency hides behind FP64 work of the same warp (a warp
-    // issues in order: an instruction that waits on a shuffle blocks everything behind it):
-    //   fetch(1) | in-lane pairs | for s = 1..H: { fetch(s+1) | B*B pairs of shift s | add returns of shift s-1 |
-    //   send returns of shift s } | add returns of shift H
+    // issues in order: an instruction that waits on a shuffle blocks everything behind it) and so that few values are
+    // live at once (the visitors of the next shift arrive body by body while those of the current one are used up, and
+    // the returned halves are added one body behind):
+    //   fetch(shift 1) | in-lane pairs among bodies 1.. |
+    //   for s = 1..H, for each visitor body c: { fetch body c of shift s+1 | B pairs (my bodies x visitor c) |
+    //                                            add the returns for my body c-1 | send the returns for visitor c } |
+    //   in-lane pairs with body 0 | add the last returns
     constexpr int H = (L - 1) / 2;
     double xv[2][B][3], vv[2][B][3], mv[2][B];  // visitors, double-buffered over the shifts
-    auto fetch = [&](int s, int buf) {
+    auto fetch_body = [&](int s, int c, int buf) {
         int ls = l + s;
         if (ls >= L) ls -= L;
         const int src = base + ls;  // whose bodies visit this lane at shift s
 #pragma unroll
-        for (int c = 0; c < B; ++c) {
-#pragma unroll
-            for (int q = 0; q < 3; ++q) {
-                xv[buf][c][q] = __shfl_sync(amask, x[c][q], src);
-                vv[buf][c][q] = __shfl_sync(amask, v[c][q], src);
-            }
-            mv[buf][c] = __shfl_sync(amask, m[c], src);
+        for (int q = 0; q < 3; ++q) {
+            xv[buf][c][q] = __shfl_sync(amask, x[c][q], src);
+            vv[buf][c][q] = __shfl_sync(amask, v[c][q], src);
         }
+        mv[buf][c] = __shfl_sync(amask, m[c], src);
     };
-    if constexpr (L > 1) fetch(1, 1);
+    if constexpr (L > 1) {
+#pragma unroll
+        for (int c = 0; c < B; ++c) fetch_body(1, c, 1);
+    }
 
     // pairs inside the lane.  Order: pairs among bodies 1.. first, pairs with local body 0 last, so that on lane 0
     // every planet receives the star's (largest) contribution last (for L = 1 this is exactly the
     // oracle's order: planets ascending, then the star).
-#pragma unroll
-    for (int bb = 1; bb <= B; ++bb) {
-        const int b = (bb == B) ? 0 : bb;
+    auto in_lane = [&](int b) {
 #pragma unroll
         for (int c = b + 1; c < B; ++c) {
             const double r2 = pair_acc_jerk(x[b], v[b], m[b], a[b], j[b], x[c], v[c], m[c], a[c], j[c]);
-            if constexpr (TRACK) min_bits(r2min, r2, !PADDED || (l * B + c < N));
+            if constexpr (TRACK) min_hi(r2min, r2, !PADDED || (l * B + c < N));
         }
-    }
+    };
+#pragma unroll
+    for (int b = 1; b < B; ++b) in_lane(b);
 
     if constexpr (L > 1) {
-        double ra[B][3], rj[B][3];  // the other half of MY bodies' pairs, computed by lane l - s
+        double ra[3], rj[3];  // the other half of the pairs of ONE of my bodies, computed by lane l - s; in flight
+        auto add_returns = [&](int body) {
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                a[body][q] += ra[q];
+                j[body][q] += rj[q];
+            }
+        };
 #pragma unroll
         for (int s = 1; s <= H; ++s) {
             const int buf = s & 1;
-            if (s < H) fetch(s + 1, buf ^ 1);
             int ls = l + s;
             if (ls >= L) ls -= L;
             int lr = l - s;
             if (lr < 0) lr += L;
             const int ret = base + lr;
-            double av[B][3], jv[B][3];
 #pragma unroll
             for (int c = 0; c < B; ++c) {
-#pragma unroll
-                for (int q = 0; q < 3; ++q) av[c][q] = jv[c][q] = 0.0;
+                if (s < H) fetch_body(s + 1, c, buf ^ 1);
+                double av[3] = {0.0, 0.0, 0.0}, jv[3] = {0.0, 0.0, 0.0};
                 const bool vvalid = !PADDED || (ls * B + c < N);
 #pragma unroll
                 for (int b = 0; b < B; ++b) {
                     const double r2 = pair_acc_jerk(x[b], v[b], m[b], a[b], j[b], xv[buf][c], vv[buf][c], mv[buf][c],
-                                                    av[c], jv[c]);
-                    if constexpr (TRACK) min_bits(r2min, r2, vvalid && (!PADDED || (l * B + b < N)));
+                                                    av, jv);
+                    if constexpr (TRACK) min_hi(r2min, r2, vvalid && (!PADDED || (l * B + b < N)));
                 }
-            }
-            if (s > 1) {
-#pragma unroll
-                for (int c = 0; c < B; ++c)
-#pragma unroll
-                    for (int q = 0; q < 3; ++q) {
-                        a[c][q] += ra[c][q];
-                        j[c][q] += rj[c][q];
-                    }
-            }
-#pragma unroll
-            for (int c = 0; c < B; ++c)
+                if (c > 0) add_returns(c - 1);  // sent one visitor body ago
+                else if (s > 1) add_returns(B - 1);
 #pragma unroll
                 for (int q = 0; q < 3; ++q) {
-                    ra[c][q] = __shfl_sync(amask, av[c][q], ret);
-                    rj[c][q] = __shfl_sync(amask, jv[c][q], ret);
+                    ra[q] = __shfl_sync(amask, av[q], ret);
+                    rj[q] = __shfl_sync(amask, jv[q], ret);
                 }
-        }
-#pragma unroll
-        for (int c = 0; c < B; ++c)
-#pragma unroll
-            for (int q = 0; q < 3; ++q) {
-                a[c][q] += ra[c][q];
-                j[c][q] += rj[c][q];
             }
+        }
+        in_lane(0);
+        add_returns(B - 1);
+    } else {
+        in_lane(0);
     }
 }
 
@@ -215,11 +214,16 @@ __device__ __forceinline__ double adaptive_dt(const double (&a)[B][3], const dou
 }
 
 // bits: 1 = close approach, 2 = ejection, 4 = non-finite position; OR-reduced over the lanes of the system.
+// r2min_hi = smallest high word of the squared pair separations this lane saw.  r^2 < r_close^2 (the exact 64-bit test,
+// R11) follows from the high words alone unless the two are equal; then (only then: the minimum separation is within
+// 2^-20 of the threshold) the systems concerned recompute the exact minimum from the positions, which are the ones
+// the evaluation used, in the same arithmetic.
 template <int N, int L, int B>
-__device__ __forceinline__ int monitor_flags(const double (&x)[B][3], u64 r2min, const StepArgs& p, int l, int base,
-                                             unsigned amask) {
+__device__ __forceinline__ int monitor_flags(const double (&x)[B][3], unsigned r2min_hi, const StepArgs& p, int l,
+                                             int base, unsigned amask) {
     constexpr bool PADDED = (L * B != N);
-    int f = (r2min < p.rc2_bits) ? 1 : 0;
+    const unsigned rc_hi = (unsigned)(p.rc2_bits >> 32);
+    int f = (r2min_hi < rc_hi) ? 1 : (r2min_hi == rc_hi) ? 8 : 0;
 #pragma unroll
     for (int b = 0; b < B; ++b) {
         const double d2 = fma(x[b][2], x[b][2], fma(x[b][1], x[b][1], x[b][0] * x[b][0]));
@@ -229,17 +233,29 @@ __device__ __forceinline__ int monitor_flags(const double (&x)[B][3], u64 r2min,
             if (db > 0x7FEFFFFFFFFFFFFFull) f |= 4;  // > DBL_MAX: +inf or NaN
         }
     }
-    if constexpr (L > 1) {
-        int g = f;
+    auto reduce = [&](int v, unsigned mask) {
+        if constexpr (L > 1) {
+            int g = v;
 #pragma unroll
-        for (int i = 1; i < L; ++i) {
-            int li = l + i;
-            if (li >= L) li -= L;
-            g |= __shfl_sync(amask, f, base + li);
+            for (int i = 1; i < L; ++i) {
+                int li = l + i;
+                if (li >= L) li -= L;
+                g |= __shfl_sync(mask, v, base + li);
+            }
+            return g;
+        } else {
+            return v;
         }
-        f = g;
+    };
+    f = reduce(f, amask);
+    const bool tie = (f & 9) == 8;  // the same for every lane of a system
+    unsigned tmask = amask;
+    if constexpr (L > 1) tmask = __ballot_sync(amask, tie);
+    if (tie) {
+        const int c = pair_r2min<N, L, B>(x, l, base, tmask) < p.rc2_bits ? 1 : 0;
+        f |= reduce(c, tmask);
     }
-    return f;
+    return f & 7;
 }
 
 // UNROLL = true: the three evaluations of a step are three inlined copies (straight-line step, best for small
@@ -372,7 +388,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
 
     double Cx[B][3], Cv[B][3];
     double a[B][3], j[B][3];
-    u64 r2min;
+    unsigned r2min;  // high word of the smallest squared pair separation seen by the last tracking evaluation
 
     // phase 0 of the loop below; returns with `active` updated.  X, V hold the accepted state.
     auto accept_and_predict = [&](unsigned amask) {
@@ -454,7 +470,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 if (!CARRY || fresh)
                     eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
                 else
-                    r2min = p.rc2_bits ? pair_r2min<N, L, B>(X, l, base, amask) : ~0ull;
+                    r2min = p.rc2_bits ? (unsigned)(pair_r2min<N, L, B>(X, l, base, amask) >> 32) : ~0u;
                 accept_and_predict(amask);
                 // lanes that just stopped take no part in the shuffles of the corrector evaluations
                 unsigned am2 = amask;
@@ -488,7 +504,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 if (!CARRY || fresh || phase != 0)
                     eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
                 else
-                    r2min = p.rc2_bits ? pair_r2min<N, L, B>(X, l, base, amask) : ~0ull;
+                    r2min = p.rc2_bits ? (unsigned)(pair_r2min<N, L, B>(X, l, base, amask) >> 32) : ~0u;
                 if (phase == 0) {
                     accept_and_predict(amask);
                 } else {

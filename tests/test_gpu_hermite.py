@@ -340,3 +340,33 @@ def test_two_million_systems_sampled_parity():
         assert (g["status"] == ens.DONE_STEPS).all() and (g["nsteps"] == 60).all()
         assert rel_diff(g["pos"][idx], o["pos"]).max() <= 1e-12 and rel_diff(g["vel"][idx], o["vel"]).max() <= 1e-12
         assert np.abs(g["time"][idx] / o["time"] - 1).max() <= 1e-13
+
+
+@pytest.mark.parametrize("n_body", [3, 10, 15])
+def test_close_approach_decided_inside_the_high_word_tie_window(n_body):
+    """The kernel tracks the minimum pair separation by the HIGH WORD of r^2 and recomputes the exact 64-bit minimum only
+    when that word equals the threshold's (hermite_kernel.cuh: monitor_flags).  Thresholds placed 2^-24 (relative, in
+    r^2) above / below the separation a system reaches at a known step put the decision inside that tie window: well
+    outside R12's 1e-9 knife edge, so (status, stop step) must equal the oracle's exactly, for every system."""
+    n_sys, dt, steps = 64, 0.002, 400
+    pos, vel, mass = _random_systems(n_sys, n_body, 900 + n_body)
+    # body n-1 of every system starts close to body 1 and approaches it (in most systems monotonically over the run)
+    for s in range(n_sys):
+        d = np.array([0.08 + 0.0005 * s, 0.004, 0.001])
+        pos[s, n_body - 1] = pos[s, 1] + d
+        vel[s, n_body - 1] = vel[s, 1] - 0.09 * d / np.linalg.norm(d)
+    free = oracle.integrate(oracle.HERMITE, pos, vel, mass, dt=dt, max_steps=150)
+    d2 = ((free["pos"][:, n_body - 1] - free["pos"][:, 1]) ** 2).sum(axis=1)  # separation^2 after 150 steps
+    hits = decided = 0
+    for s in range(0, n_sys, 7):
+        for sign in (+1.0, -1.0):
+            rc = float(np.sqrt(d2[s] * (1.0 + sign * 2.0**-24)))
+            hi = lambda x: np.float64(x).view(np.uint64) >> np.uint64(32)
+            g = ens.run(ens.HERMITE, pos, vel, mass, dt=dt, steps=steps, r_close=rc)
+            o = oracle.integrate(oracle.HERMITE, pos, vel, mass, dt=dt, max_steps=steps, r_close=rc)
+            assert (g["status"] == o["status"]).all() and (g["nsteps"] == o["nsteps"]).all(), (s, sign)
+            assert o["status"][s] == oracle.STOP_CLOSE
+            # threshold just above the separation of step 150: stop there; just below: one step later
+            decided += int(o["nsteps"][s] == (150 if sign > 0 else 151))
+            hits += int(hi(d2[s]) == hi(rc * rc))
+    assert hits >= 10 and decided >= 8  # the cases really sit in the tie window and it decides the stop step
