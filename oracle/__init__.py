@@ -24,8 +24,10 @@ _LIB = os.path.join(_HERE, "libens_oracle.so")
 _lock = threading.Lock()
 _lib = None
 
-ACTIVE, DONE_TIME, DONE_STEPS, STOP_CLOSE, STOP_EJECT, STOP_NONFINITE = range(6)
-HERMITE, MVS, HERMITE_ADAPTIVE, HERMITE_CARRY, RKCK = 0, 1, 2, 3, 4
+ACTIVE, DONE_TIME, DONE_STEPS, STOP_CLOSE, STOP_EJECT, STOP_NONFINITE, STOP_STEPSIZE = range(7)
+HERMITE, MVS, HERMITE_ADAPTIVE, HERMITE_CARRY, RKCK, MVS_MERGED, RKCK_ADAPTIVE = 0, 1, 2, 3, 4, 5, 6
+# MVS_MERGED: the adjacent half drifts / half kicks of consecutive steps merged.  RKCK_ADAPTIVE: `dt` is the first trial
+# step, `rk_eps` the accuracy parameter (reading R-RK2').
 # HERMITE_ADAPTIVE: `dt` is the step size scale tau of Eq. 5.  HERMITE_CARRY: Alg. 2 as printed, 2 evaluations per step.
 DOUBLE, LONG_DOUBLE = 0, 1
 
@@ -53,6 +55,8 @@ def _load():
         lib.orc_acc_jerk.argtypes = [ci, d, d, d, d, d, ci]
         lib.orc_hermite_step.argtypes = [ci, d, d, d, cd, ci, ci]
         lib.orc_integrate.argtypes = [ci, cl, ci, d, d, d, d, i32, i64, cd, cd, cl, cd, cd, ci, ci]
+        lib.orc_integrate2.argtypes = [ci, cl, ci, d, d, d, d, i32, i64, cd, cd, cl, cd, cd, ci, ci, cd, i64]
+        lib.orc_rkck_adaptive_trial.argtypes = [ci, d, d, d, d, cd, d, ctypes.POINTER(ci), ci]
         lib.orc_adaptive_dt.argtypes = [ci, d, d, d, cd, d, ci]
         lib.orc_rkck_step.argtypes = [ci, d, d, d, cd, d, d, ci]
         lib.orc_rkck_tableau.argtypes = [d, d, d, d]
@@ -123,9 +127,18 @@ def adaptive_dt(x, v, m, tau, prec=DOUBLE):
     return float(out[0])
 
 
+def rkck_adaptive_trial(x, v, m, h, eps, prec=DOUBLE):
+    """One trial step of the adaptive Cash-Karp integrator (R-RK2'): returns (x, v, h_next, r, accepted)."""
+    x, v, m = _f64(x).copy(), _f64(v).copy(), _f64(m)
+    hh, r, ok = np.array([float(h)]), np.zeros(1), ctypes.c_int(0)
+    rc = _load().orc_rkck_adaptive_trial(m.shape[0], _p(x), _p(v), _p(m), _p(hh), float(eps), _p(r), ctypes.byref(ok), prec)
+    assert rc == 0
+    return x, v, float(hh[0]), float(r[0]), bool(ok.value)
+
+
 def integrate(integrator, pos, vel, mass, time=None, *, dt, t_end=np.inf, max_steps, r_close=0.0, r_eject=np.inf,
-              status=None, nsteps=None, prec=DOUBLE, nthreads=None):
-    """Alg. 1 over an ensemble.  Returns dict(pos, vel, time, status, nsteps) (new arrays)."""
+              status=None, nsteps=None, prec=DOUBLE, nthreads=None, rk_eps=1e-9):
+    """Alg. 1 over an ensemble.  Returns dict(pos, vel, time, status, nsteps, nreject) (new arrays)."""
     pos, vel, mass = _f64(pos).copy(), _f64(vel).copy(), _f64(mass)
     n_sys, n = mass.shape
     assert pos.shape == (n_sys, n, 3) and vel.shape == (n_sys, n, 3)
@@ -134,13 +147,15 @@ def integrate(integrator, pos, vel, mass, time=None, *, dt, t_end=np.inf, max_st
     nsteps = np.zeros(n_sys, np.int64) if nsteps is None else np.ascontiguousarray(nsteps, np.int64).copy()
     if nthreads is None:
         nthreads = host_cores()
-    rc = _load().orc_integrate(
+    nreject = np.zeros(n_sys, np.int64)
+    rc = _load().orc_integrate2(
         int(integrator), n_sys, n, _p(pos), _p(vel), _p(mass), _p(time),
         status.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), nsteps.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)),
-        float(dt), float(t_end), int(max_steps), float(r_close), float(r_eject), prec, int(nthreads))
+        float(dt), float(t_end), int(max_steps), float(r_close), float(r_eject), prec, int(nthreads), float(rk_eps),
+        nreject.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)))
     if rc != 0:
         raise ValueError("oracle: bad arguments")
-    return dict(pos=pos, vel=vel, time=time, status=status, nsteps=nsteps)
+    return dict(pos=pos, vel=vel, time=time, status=status, nsteps=nsteps, nreject=nreject)
 
 
 def energy(pos, vel, mass, prec=DOUBLE):

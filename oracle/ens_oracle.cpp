@@ -17,8 +17,13 @@
 // closed forms, test-particle exactness of the Kepler drift, hand-built monitor crossings; adaptive step (Eq. 5):
 // circular and apsidal closed forms dt = tau / (w sqrt 2), scaling laws, order 4 in tau; 2-evaluation Hermite: order
 // 4, first step identical to the 3-evaluation step; Cash-Karp: all 17 rooted-tree order conditions on the tableau,
-// measured order 5 (embedded: 4).  No function in this file is "parity unpinned"; the only unpinned item is the
-// paper's Table 1, whose orbital phases are unspecified.
+// measured order 5 (embedded: 4); the Kepler solver's bracket-and-bisect fallback: cases that reach it against Kepler's
+// equation (elliptic, multi-revolution) and against orbit invariants, the hyperbolic Kepler equation and the group
+// property (hyperbolic); adaptive Cash-Karp: convergence to Kepler's equation at the rate the control implies, the
+// control's definition on single trial steps, rejected steps leaving the state untouched; merged MVS: one step
+// bit-identical to the unmerged step, same order-2 convergence and invariants.  The whole file runs clean under
+// AddressSanitizer + UBSan (tests/test_oracle_sanitize.py).  No function in this file is "parity unpinned"; the only
+// unpinned item is the paper's Table 1, whose orbital phases are unspecified.
 
 #include <cmath>
 #include <cstdint>
@@ -28,7 +33,7 @@
 
 namespace {
 
-enum { ST_ACTIVE = 0, ST_DONE_TIME = 1, ST_DONE_STEPS = 2, ST_STOP_CLOSE = 3, ST_STOP_EJECT = 4, ST_STOP_NONFINITE = 5 };
+enum { ST_ACTIVE = 0, ST_DONE_TIME = 1, ST_DONE_STEPS = 2, ST_STOP_CLOSE = 3, ST_STOP_EJECT = 4, ST_STOP_NONFINITE = 5, ST_STOP_STEPSIZE = 6 };
 
 template <class R> inline R rsqrt_exact(R r2) { return R(1) / std::sqrt(r2); }
 
@@ -490,13 +495,75 @@ void mvs_step(DH<R>& s, const R* m, R h) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Adaptive-step Runge-Kutta Cash-Karp ("closely based on the gsl_odeiv2_step_rkck stepper ... one with an
+// adaptive time-step"; "uses the Cash-Karp method at the end of the step to compute the 5th order error.  If
+// the error exceeds the user specified accuracy parameter (eps), the step is rejected, e.g. positions, velocities and
+// time are not updated ...  Instead, the next attempted time-step will use a smaller time-step").  The paper gives
+// neither the error norm nor the step-size rule; reading R-RK2' takes the standard step-size
+// control the GSL manual documents for that stepper family:
+//   error level of a trial step   r = max( max|errx| / (eps X),  max|errv| / (eps V) ),   err = y5 - y4 of rkck_step,
+//                                 X = max_b |x_b|_2, V = max_b |v_b|_2 of the state the step starts from (the scale of
+//                                 reading R13; a per-component relative scale is undefined for the exact zeros of
+//                                 coplanar initial conditions);
+//   r > 1.1   reject: state and time untouched, h <- h max(1/5, F(S r^(-1/q))), try again;
+//   else      accept (the fifth-order solution, R-RK1; t += h), and if r < 0.5 the NEXT step starts from
+//             h <- h min(5, max(1, F(S r^(-1/(q+1)))));
+//   S = 0.9, q = 4 (the manual's "consistency order, e.g. q = 4 for 4(5) embedded RK");
+//   F(f) = floor(16 f) / 16: the factor is taken from a discrete set (the device the paper proposes for reproducible
+//   adaptive steps, "choose from a discrete set of time steps").  The error estimate is a difference of nearly
+//   equal sums, so r carries relative rounding noise of 1e-9..1e-7; with a continuous factor that noise would reach
+//   every later step size and time, and two correct implementations would differ at the 1e-8 level after a few
+//   hundred steps; with the discrete factor they take bit-identical steps unless r falls within the noise of a
+//   boundary (rare, and then both step sequences are valid).
+// h is the per-system trial step; every call starts it at the caller's dt (sign = direction).  No clipping of the
+// last step (R10).  *accepted: 1 if the step was taken.  Returns the error level r.
+// ---------------------------------------------------------------------------------------------------
+template <class R>
+R rkck_adaptive_trial(int n, R* x, R* v, const R* m, R& h, R eps, bool* accepted) {
+    const int d = 3 * n;
+    std::vector<R> xn(x, x + d), vn(v, v + d), ex(d), ev(d);
+    rkck_step(n, xn.data(), vn.data(), m, h, ex.data(), ev.data());
+    R X = 0, V = 0, EX = 0, EV = 0;
+    for (int i = 0; i < n; ++i) {
+        const R xx = std::sqrt(x[3 * i] * x[3 * i] + x[3 * i + 1] * x[3 * i + 1] + x[3 * i + 2] * x[3 * i + 2]);
+        const R vv = std::sqrt(v[3 * i] * v[3 * i] + v[3 * i + 1] * v[3 * i + 1] + v[3 * i + 2] * v[3 * i + 2]);
+        if (xx > X) X = xx;
+        if (vv > V) V = vv;
+    }
+    for (int q = 0; q < d; ++q) {
+        if (std::fabs(ex[q]) > EX) EX = std::fabs(ex[q]);
+        if (std::fabs(ev[q]) > EV) EV = std::fabs(ev[q]);
+    }
+    const R rx = EX / (eps * X), rv = EV / (eps * V);
+    const R r = rx > rv ? rx : rv;
+    const R S = R(9) / R(10);
+    if (r > R(11) / R(10)) {  // reject: nothing but h changes
+        R f = std::floor(R(16) * (S * std::pow(r, R(-1) / R(4)))) / R(16);
+        if (f < R(1) / R(5)) f = R(1) / R(5);
+        h *= f;
+        *accepted = false;
+        return r;
+    }
+    for (int q = 0; q < d; ++q) { x[q] = xn[q]; v[q] = vn[q]; }
+    *accepted = true;
+    if (r < R(1) / R(2)) {
+        R f = std::floor(R(16) * (S * std::pow(r, R(-1) / R(5)))) / R(16);
+        if (f > R(5)) f = R(5);
+        if (f < R(1)) f = R(1);
+        h *= f;  // r = 0 gives f = inf -> 5
+    }
+    return r;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // The generic integrator loop, Alg. 1 with R10-R12:
 //   while ACTIVE and steps_this_call < max_steps and time left: advance; ++nsteps; t += h; monitors;
 //   exit status: STOP_* (sticky) | DONE_TIME (t reached t_end) | DONE_STEPS.
 // ---------------------------------------------------------------------------------------------------
 template <class R>
 void run_system(int integrator, int n, double* pos, double* vel, const double* mass, double* time, int32_t* status,
-                int64_t* nsteps, double dt, double t_end, int64_t max_steps, double r_close, double r_eject, int n_corr) {
+                int64_t* nsteps, double dt, double t_end, int64_t max_steps, double r_close, double r_eject, int n_corr,
+                double rk_eps = 1e-9, int64_t* nreject = nullptr) {
     if (*status >= ST_STOP_CLOSE) return;  // sticky until the state is set again
     std::vector<R> x(3 * n), v(3 * n), m(n);
     for (int q = 0; q < 3 * n; ++q) { x[q] = pos[q]; v[q] = vel[q]; }
@@ -509,16 +576,74 @@ void run_system(int integrator, int n, double* pos, double* vel, const double* m
     std::vector<R> xm(3 * n), ca(3 * n), cj(3 * n);
     if (integrator == 3)  // carried (a, j): evaluated once at the state the call starts from
         eval_acc_jerk(n, x.data(), v.data(), m.data(), ca.data(), cj.data());
-    if (integrator == 1) {
+    if (integrator == 1 || integrator == 5) {
         to_dh(n, x.data(), v.data(), m.data(), s);
         eval_acc_planets(n, s.Q.data(), m.data(), s.A.data());  // prepare(P)
     }
+    if (integrator == 5) {
+        // MVS with the adjacent half sub-steps of consecutive steps merged (P:L105-109 lists five sub-steps; P:L256:
+        // "the separation between planets does not change during Cartesian drift and kick sub-steps").  The closing
+        // half drift of step k and the opening one of step k+1 use the same drift velocity and are one full drift; the
+        // kick commutes with the Cartesian drift (the planets' accelerations sum to zero momentum, so the drift velocity
+        // is the same before and after a kick, and the drift moves every planet alike, so A is unchanged): the two half
+        // kicks that surround the merged drift are one full kick.  In exact arithmetic every post-step state equals the
+        // unmerged map's; rounding differs (the "parity cost", measured in tests/test_oracle_mvs_merged.py).
+        //   open:  D(h/2) K(h/2)
+        //   step:  Kepler(h); A = acc;  post-step state = K(h/2) D(h/2) of the current one (formed for the monitors
+        //          and as the result when the loop ends here);  if the loop goes on: K(h) D(h) instead.
+        const R hh = h / R(2);
+        bool opened = false;
+        DH<R> post;
+        while (true) {
+            if (!time_left(dt, (double)t, t_end)) { st = ST_DONE_TIME; break; }
+            if (k >= max_steps) { st = ST_DONE_STEPS; break; }
+            if (!opened) {
+                mvs_linear_drift(s, m.data(), hh);
+                mvs_kick(s, hh);
+                opened = true;
+            }
+            for (int i = 1; i < n; ++i) kepler_drift(&s.Q[3 * i], &s.V[3 * i], m[0], h);
+            eval_acc_planets(n, s.Q.data(), m.data(), s.A.data());
+            post = s;  // closing halves on a copy: the state Alg. 1 shows the monitors (and the caller)
+            mvs_kick(post, hh);
+            mvs_linear_drift(post, m.data(), hh);
+            t += h;
+            ++k;
+            from_dh<R>(post, m.data(), xm.data(), nullptr);
+            const int mon = monitors(n, xm.data(), r_close, r_eject);
+            if (mon != ST_ACTIVE) { st = mon; break; }
+            if (!time_left(dt, (double)t, t_end) || k >= max_steps) continue;  // the loop head ends the run: no merge
+            mvs_kick(s, h);                      // K(h/2) of this step + K(h/2) of the next
+            mvs_linear_drift(s, m.data(), h);    // D(h/2) of this step + D(h/2) of the next (drift velocity after the kick)
+        }
+        if (k > 0) s = post;
+        from_dh(s, m.data(), x.data(), v.data());
+        for (int q = 0; q < 3 * n; ++q) { pos[q] = (double)x[q]; vel[q] = (double)v[q]; }
+        *time = (double)t;
+        *status = st;
+        *nsteps += k;
+        return;
+    }
+    R htrial = h;       // integrator 6: the per-system trial step, started at dt by every call
+    int64_t nrej = 0;
     while (true) {
         if (!time_left(dt, (double)t, t_end)) { st = ST_DONE_TIME; break; }
         if (k >= max_steps) { st = ST_DONE_STEPS; break; }
         const R* xmon;
         R hs = h;  // the step actually taken (t += hs below)
-        if (integrator == 0) {
+        if (integrator == 6) {  // adaptive Runge-Kutta Cash-Karp: trial steps until one is accepted
+            bool ok = false;
+            bool underflow = false;
+            while (true) {
+                hs = htrial;
+                rkck_adaptive_trial(n, x.data(), v.data(), m.data(), htrial, (R)rk_eps, &ok);
+                if (ok) break;
+                ++nrej;
+                if (t + htrial == t) { underflow = true; break; }  // the step can no longer advance the time
+            }
+            if (underflow) { st = ST_STOP_STEPSIZE; break; }
+            xmon = x.data();
+        } else if (integrator == 0) {
             hermite_step(n, x.data(), v.data(), m.data(), h, n_corr);
             xmon = x.data();
         } else if (integrator == 4) {  // fixed-step Runge-Kutta Cash-Karp
@@ -546,6 +671,7 @@ void run_system(int integrator, int n, double* pos, double* vel, const double* m
     *time = (double)t;
     *status = st;
     *nsteps += k;
+    if (nreject) *nreject += nrej;
 }
 
 }  // namespace
@@ -583,22 +709,53 @@ int orc_hermite_step(int n, double* x, double* v, const double* m, double h, int
 // integrator: 0 = Hermite (fixed step dt), 1 = MVS, 2 = adaptive Hermite (dt = tau of Eq. 5),
 // 3 = Hermite with 2 evaluations per step (Alg. 2 as printed; a, j carried from step to step),
 // 4 = fixed-step Runge-Kutta Cash-Karp (fifth-order solution propagated).  status/nsteps/time are in-out ([n_sys]); status STOP_* is sticky.
-int orc_integrate(int integrator, int64_t n_sys, int n, double* pos, double* vel, const double* mass, double* time,
-                  int32_t* status, int64_t* nsteps, double dt, double t_end, int64_t max_steps, double r_close,
-                  double r_eject, int prec, int nthreads) {
+// 5 = MVS with merged half sub-steps, 6 = adaptive Runge-Kutta Cash-Karp (dt = first trial step, rk_eps = accuracy
+// parameter; nreject [n_sys] in-out or NULL receives the rejected trial steps).
+int orc_integrate2(int integrator, int64_t n_sys, int n, double* pos, double* vel, const double* mass, double* time,
+                   int32_t* status, int64_t* nsteps, double dt, double t_end, int64_t max_steps, double r_close,
+                   double r_eject, int prec, int nthreads, double rk_eps, int64_t* nreject) {
     if (n_sys < 0 || n < 2 || !pos || !vel || !mass || !time || !status || !nsteps) return -1;
-    if (!(dt != 0) || !std::isfinite(dt) || max_steps < 0 || (integrator < 0 || integrator > 4)) return -1;
+    if (!(dt != 0) || !std::isfinite(dt) || max_steps < 0 || (integrator < 0 || integrator > 6)) return -1;
+    if (integrator == 6 && !(rk_eps > 0)) return -1;
     if (nthreads < 1) nthreads = 1;
 #pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads)
     for (int64_t s = 0; s < n_sys; ++s) {
         double* p = pos + s * 3 * n;
         double* w = vel + s * 3 * n;
         const double* mm = mass + s * n;
+        int64_t* nr = nreject ? nreject + s : nullptr;
         if (prec == 0)
-            run_system<double>(integrator, n, p, w, mm, time + s, status + s, nsteps + s, dt, t_end, max_steps, r_close, r_eject, 2);
+            run_system<double>(integrator, n, p, w, mm, time + s, status + s, nsteps + s, dt, t_end, max_steps, r_close, r_eject, 2, rk_eps, nr);
         else
-            run_system<long double>(integrator, n, p, w, mm, time + s, status + s, nsteps + s, dt, t_end, max_steps, r_close, r_eject, 2);
+            run_system<long double>(integrator, n, p, w, mm, time + s, status + s, nsteps + s, dt, t_end, max_steps, r_close, r_eject, 2, rk_eps, nr);
     }
+    return 0;
+}
+
+int orc_integrate(int integrator, int64_t n_sys, int n, double* pos, double* vel, const double* mass, double* time,
+                  int32_t* status, int64_t* nsteps, double dt, double t_end, int64_t max_steps, double r_close,
+                  double r_eject, int prec, int nthreads) {
+    if (integrator < 0 || integrator > 4) return -1;
+    return orc_integrate2(integrator, n_sys, n, pos, vel, mass, time, status, nsteps, dt, t_end, max_steps, r_close,
+                          r_eject, prec, nthreads, 1e-9, nullptr);
+}
+
+// one trial step of the adaptive Cash-Karp integrator on one system (test hook): x, v, *h in-out; *r = error level,
+// *accepted = 1 if the step was taken (then x, v hold the new state and *h the next trial step)
+int orc_rkck_adaptive_trial(int n, double* x, double* v, const double* m, double* h, double eps, double* r, int* accepted,
+                            int prec) {
+    if (n < 2 || !x || !v || !m || !h || !r || !accepted || !(eps > 0)) return -1;
+    bool ok = false;
+    if (prec == 0) {
+        *r = rkck_adaptive_trial<double>(n, x, v, m, *h, eps, &ok);
+    } else {
+        std::vector<long double> X(x, x + 3 * n), V(v, v + 3 * n), M(m, m + n);
+        long double H = *h;
+        *r = (double)rkck_adaptive_trial<long double>(n, X.data(), V.data(), M.data(), H, (long double)eps, &ok);
+        for (int q = 0; q < 3 * n; ++q) { x[q] = (double)X[q]; v[q] = (double)V[q]; }
+        *h = (double)H;
+    }
+    *accepted = ok ? 1 : 0;
     return 0;
 }
 
