@@ -43,7 +43,11 @@ extern "C" {
 typedef struct ens ens_t; /* opaque */
 
 enum { ENS_OK = 0, ENS_EINVAL = -1, ENS_ENOMEM = -2, ENS_ECUDA = -3, ENS_ESTATE = -4, ENS_EUNSUPPORTED = -5 };
-enum { ENS_HERMITE = 0, ENS_MVS = 1, ENS_HERMITE_ADAPTIVE = 2, ENS_HERMITE_CARRY = 3, ENS_RKCK = 4 };
+enum {
+    ENS_HERMITE = 0, ENS_MVS = 1, ENS_HERMITE_ADAPTIVE = 2, ENS_HERMITE_CARRY = 3, ENS_RKCK = 4,
+    ENS_MVS_MERGED = 5,    /* MVS with the adjacent half sub-steps of consecutive steps merged */
+    ENS_RKCK_ADAPTIVE = 6  /* Cash-Karp with step rejection and step-size control (R-RK2') */
+};
 enum { ENS_HOST = 0, ENS_DEVICE = 1 };
 /* per-system status (Alg. 1 "state").  DONE_* become ACTIVE again at the next ens_integrate;
  * STOP_* are sticky until ens_set_state. */
@@ -53,7 +57,8 @@ enum {
     ENS_DONE_STEPS = 2,     /* max_steps taken in this call (Alg. 1 max-iterations) */
     ENS_STOP_CLOSE = 3,     /* some pair separation < r_close after a step (monitor; R11) */
     ENS_STOP_EJECT = 4,     /* some body farther than r_eject from the coordinate origin after a step (R11) */
-    ENS_STOP_NONFINITE = 5  /* a position became non-finite */
+    ENS_STOP_NONFINITE = 5, /* a position became non-finite */
+    ENS_STOP_STEPSIZE = 6   /* adaptive Runge-Kutta: the rejected step shrank until t + h == t (tolerance unreachable) */
 };
 
 /* Create an ensemble of n_sys >= 1 systems of 2 <= n_body <= 16 bodies on the current CUDA device and
@@ -81,6 +86,14 @@ ENS_API int ens_set_state(ens_t *e, const double *pos, const double *vel, const 
  * EINVAL: NULL handle or NaN. */
 ENS_API int ens_set_monitors(ens_t *e, double r_close, double r_eject);
 
+/* Accuracy parameter eps of ENS_RKCK_ADAPTIVE ("user specified accuracy parameter"; default 1e-9): a trial step
+ * is accepted when max(max|err_x| / (eps X), max|err_v| / (eps V)) <= 1.1, X and V the largest body distance and speed
+ * of the system at the start of the step.  EINVAL: NULL handle, eps <= 0 or non-finite. */
+ENS_API int ens_set_rk_tolerance(ens_t *e, double eps);
+
+/* Rejected trial steps per system since ens_set_state (ENS_RKCK_ADAPTIVE), int64 [n_sys].  ESTATE: no state. */
+ENS_API int ens_get_rejected(const ens_t *e, int64_t *nreject, int memspace, void *stream);
+
 /* Advance every system independently (Alg. 1), entirely on the device, in ONE kernel launch
  * with the state resident in registers across all steps:
  *     while status == ACTIVE && steps_this_call < max_steps && time left:  step(dt); t += dt; ++nsteps; monitors
@@ -95,7 +108,15 @@ ENS_API int ens_set_monitors(ens_t *e, double r_close, double r_eject);
  * (reading R6-alt): fixed step, TWO evaluations per step, a^(0), j^(0) of a step being the a^(2), j^(2)
  * the previous step left behind (only the first step of a call evaluates at the state itself, so a run split over
  * two calls is not bit-identical to the unsplit one); ENS_RKCK = fixed-step Runge-Kutta Cash-Karp (P:L93-97,
- * P:L246-248): six acceleration evaluations per step, no jerk, the fifth-order solution propagated (R-RK1).
+ * P:L246-248): six acceleration evaluations per step, no jerk, the fifth-order solution propagated (R-RK1);
+ * ENS_MVS_MERGED = the MVS map with the closing half drift / half kick of a step and the opening ones of the next
+ * merged into a full kick and a full drift (the same map in exact arithmetic; rounding-level differences from ENS_MVS;
+ * a run split over two calls closes and re-opens the half sub-steps); ENS_RKCK_ADAPTIVE = Cash-Karp with the embedded
+ * error estimate controlling the step (reading R-RK2' of DESIGN.md section 3: the GSL manual's standard
+ * control, step factors floor(16 f)/16): `dt` is the first trial step of every system (its sign gives the direction),
+ * ens_set_rk_tolerance gives the accuracy parameter eps, a trial step whose error level exceeds 1.1 is rejected (state
+ * and time untouched, counted in ens_get_rejected) and retried with a smaller step, `max_steps` counts accepted steps,
+ * and a system whose step shrinks until t + h == t stops with ENS_STOP_STEPSIZE.
  * EINVAL: NULL handle, unknown integrator, dt == 0 or non-finite, NaN t_end, max_steps < 0.
  * ESTATE: no state was set.  ECUDA: launch failed. */
 ENS_API int ens_integrate(ens_t *e, int integrator, double dt, double t_end, int64_t max_steps, void *stream);

@@ -138,6 +138,7 @@ __global__ void __launch_bounds__(256) pack_state_kernel(const double* __restric
         e.time[i] = (threadIdx.x < nv && time_src) ? time_src[i] : 0.0;
         e.status[i] = ENS_ACTIVE;
         e.nsteps[i] = 0;
+        e.nreject[i] = 0;
     }
 }
 
@@ -317,6 +318,7 @@ __global__ void log_reset_kernel(int64_t* last, int64_t n, unsigned long long* c
 struct ens {
     ensd::View v{};
     double r_close = 0.0, r_eject = INFINITY;
+    double rk_eps = 1e-9;
     bool have_state = false;
     int device = 0;
     // device staging (AoS) for host-space calls, allocated by the first host-space call (which waits for the stream
@@ -324,7 +326,7 @@ struct ens {
     // (a lazily filled cache: the read-only calls may fill it too, hence mutable)
     mutable double* stage = nullptr;        // [n_sys * n_body * 7] : pos | vel | mass
     mutable double* stage_small = nullptr;  // [n_sys * 4] : time / E | L
-    ensd::KernelInfo hermite{}, hermite_sliced{}, hermite_adaptive{}, hermite_carry{}, rkck{}, mvs{};
+    ensd::KernelInfo hermite{}, hermite_sliced{}, hermite_adaptive{}, hermite_carry{}, rkck{}, rkck_adaptive{}, mvs{}, mvs_merged{};
     unsigned long long* counter = nullptr;  // work counter of the persistent kernels
     int32_t* slice_done = nullptr;          // per warp-group slice counters of the time-sliced Hermite kernel
     ensd::OrderBuffers order;               // hand-out order of the adaptive kernels (allocated by ens_create)
@@ -414,6 +416,7 @@ int ens_create(int64_t n_sys, int n_body, ens_t** out) {
     alloc((void**)&e->v.time, sizeof(double) * np);
     alloc((void**)&e->v.status, sizeof(int32_t) * np);
     alloc((void**)&e->v.nsteps, sizeof(int64_t) * np);
+    alloc((void**)&e->v.nreject, sizeof(int64_t) * np);
     alloc((void**)&e->counter, sizeof(unsigned long long));
     alloc((void**)&e->slice_done, sizeof(int32_t) * (size_t)ensd::hermite_slice_groups(n_sys, n_body));
     // everything ens_integrate needs is allocated here: device-space calls only enqueue
@@ -429,8 +432,10 @@ int ens_create(int64_t n_sys, int n_body, ens_t** out) {
     e->hermite_adaptive = ensd::hermite_kernel_for(n_body, 1);
     e->hermite_carry = ensd::hermite_kernel_for(n_body, 2);
     e->hermite_sliced = ensd::hermite_kernel_for(n_body, 3);
-    e->rkck = ensd::rkck_kernel_for(n_body);
-    e->mvs = ensd::mvs_kernel_for(n_body);
+    e->rkck = ensd::rkck_kernel_for(n_body, false);
+    e->rkck_adaptive = ensd::rkck_kernel_for(n_body, true);
+    e->mvs = ensd::mvs_kernel_for(n_body, false);
+    e->mvs_merged = ensd::mvs_kernel_for(n_body, true);
     *out = e;
     return ENS_OK;
 }
@@ -446,6 +451,7 @@ int ens_destroy(ens_t* e) {
         cudaFree(e->v.time);
         cudaFree(e->v.status);
         cudaFree(e->v.nsteps);
+        cudaFree(e->v.nreject);
         cudaFree(e->counter);
         cudaFree(e->slice_done);
         cudaFree(e->log.cursor);
@@ -477,6 +483,23 @@ int ens_set_monitors(ens_t* e, double r_close, double r_eject) {
     if (!e || std::isnan(r_close) || std::isnan(r_eject)) return ENS_EINVAL;
     e->r_close = r_close > 0.0 ? r_close : 0.0;
     e->r_eject = r_eject > 0.0 ? r_eject : INFINITY;
+    return ENS_OK;
+}
+
+int ens_set_rk_tolerance(ens_t* e, double eps) {
+    if (!e || !(eps > 0.0) || !std::isfinite(eps)) return ENS_EINVAL;
+    e->rk_eps = eps;
+    return ENS_OK;
+}
+
+int ens_get_rejected(const ens_t* e, int64_t* nreject, int memspace, void* stream) {
+    if (!e || !nreject || (memspace != ENS_HOST && memspace != ENS_DEVICE)) return ENS_EINVAL;
+    if (!e->have_state) return ENS_ESTATE;
+    ENS_ON_DEVICE(e);
+    cudaStream_t s = (cudaStream_t)stream;
+    CU(cudaMemcpyAsync(nreject, e->v.nreject, sizeof(int64_t) * e->v.n_sys,
+                       memspace == ENS_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, s));
+    if (memspace == ENS_HOST) CU(cudaStreamSynchronize(s));
     return ENS_OK;
 }
 
@@ -512,7 +535,7 @@ int ens_set_state(ens_t* e, const double* pos, const double* vel, const double* 
 }
 
 int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max_steps, void* stream) {
-    if (!e || integrator < ENS_HERMITE || integrator > ENS_RKCK) return ENS_EINVAL;
+    if (!e || integrator < ENS_HERMITE || integrator > ENS_RKCK_ADAPTIVE) return ENS_EINVAL;
     if (!(dt != 0.0) || !std::isfinite(dt) || std::isnan(t_end) || max_steps < 0) return ENS_EINVAL;
     if (!e->have_state) return ENS_ESTATE;
     ENS_ON_DEVICE(e);
@@ -530,6 +553,8 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
     a.counter = e->counter;
     a.order = nullptr;
     a.slice_done = e->slice_done;
+    a.rk_eps = e->rk_eps;
+    if (integrator == ENS_RKCK_ADAPTIVE) CU(cudaMemsetAsync(e->counter, 0, sizeof(unsigned long long), s));
     if (integrator == ENS_HERMITE_ADAPTIVE) {
         CU(cudaMemsetAsync(e->counter, 0, sizeof(unsigned long long), s));
         if (!e->tune.adaptive_unordered && e->order.idx_out) {
@@ -542,15 +567,17 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
                                  : integrator == ENS_HERMITE_ADAPTIVE ? e->hermite_adaptive
                                  : integrator == ENS_HERMITE_CARRY    ? e->hermite_carry
                                  : integrator == ENS_RKCK             ? e->rkck
+                                 : integrator == ENS_RKCK_ADAPTIVE    ? e->rkck_adaptive
+                                 : integrator == ENS_MVS_MERGED       ? e->mvs_merged
                                                                       : e->mvs;
     if (!ki.fn) return ENS_EUNSUPPORTED;
     const int threads = e->tune.threads ? e->tune.threads : ki.threads;
     const void* fn = ki.fn;
     CU(cudaEventRecord(e->ev0, s));
-    cudaError_t err = integrator == ENS_MVS
-                          ? ensd::launch_mvs(e->v, a, threads, s, &e->last_blocks)
-                      : integrator == ENS_RKCK
-                          ? ensd::launch_rkck(e->v, a, threads, s, &e->last_blocks)
+    cudaError_t err = (integrator == ENS_MVS || integrator == ENS_MVS_MERGED)
+                          ? ensd::launch_mvs(e->v, a, integrator == ENS_MVS_MERGED, threads, s, &e->last_blocks)
+                      : (integrator == ENS_RKCK || integrator == ENS_RKCK_ADAPTIVE)
+                          ? ensd::launch_rkck(e->v, a, integrator == ENS_RKCK_ADAPTIVE, threads, s, &e->last_blocks)
                           : ensd::launch_hermite(e->v, a, integrator == ENS_HERMITE_ADAPTIVE ? 1 : integrator == ENS_HERMITE_CARRY ? 2 : 0,
                                                  e->tune, s, &e->last_blocks, &fn);
     if (err != cudaSuccess) return cuda_fail(err, "ens_integrate launch");
@@ -699,7 +726,8 @@ int ens_log_read(const ens_t* e, int64_t* n_records, int64_t* n_dropped, int64_t
 int ens_get_info(const ens_t* e, int64_t out[8]) {
     if (!e || !out) return ENS_EINVAL;
     ENS_ON_DEVICE(e);
-    const ensd::KernelInfo* all[] = {&e->mvs, &e->hermite_adaptive, &e->hermite_carry, &e->hermite_sliced, &e->rkck};
+    const ensd::KernelInfo* all[] = {&e->mvs, &e->hermite_adaptive, &e->hermite_carry, &e->hermite_sliced, &e->rkck,
+                                     &e->rkck_adaptive, &e->mvs_merged};
     const ensd::KernelInfo* ki = &e->hermite;
     for (const ensd::KernelInfo* c : all)
         if (e->last_fn && e->last_fn == c->fn) ki = c;

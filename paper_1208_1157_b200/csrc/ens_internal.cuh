@@ -18,6 +18,7 @@ struct View {
     double* time;     // [n_pad]
     int32_t* status;  // [n_pad]
     int64_t* nsteps;  // [n_pad]
+    int64_t* nreject; // [n_pad] rejected trial steps (adaptive Runge-Kutta)
     int64_t n_sys;
     int64_t n_pad;    // multiple of 64 systems -> every row starts 512-byte aligned
     int n_body;
@@ -42,6 +43,7 @@ struct StepArgs {
     // steps), handed out slice-major; slice_done[g] = slices group g has completed (zeroed before the launch)
     int32_t* slice_done;
     int64_t slice_steps, n_slices, n_groups;
+    double rk_eps;  // accuracy parameter of the adaptive Runge-Kutta integrator
 };
 
 inline void fill_step_constants(StepArgs& a) {
@@ -96,9 +98,9 @@ KernelInfo hermite_kernel_for(int n_body, int mode);  // mode: 0 fixed step, 1 a
 int64_t hermite_slice_groups(int64_t n_sys, int n_body);
 cudaError_t launch_hermite(const View& v, const StepArgs& a, int mode, const LaunchTune& tune, cudaStream_t s,
                            int64_t* blocks_out, const void** fn_out);
-KernelInfo rkck_kernel_for(int n_body);
-cudaError_t launch_rkck(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out);
-KernelInfo mvs_kernel_for(int n_body);
-cudaError_t launch_mvs(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out);
+KernelInfo rkck_kernel_for(int n_body, bool adaptive);
+cudaError_t launch_rkck(const View& v, const StepArgs& a, bool adaptive, int threads, cudaStream_t s, int64_t* blocks_out);
+KernelInfo mvs_kernel_for(int n_body, bool merged);
+cudaError_t launch_mvs(const View& v, const StepArgs& a, bool merged, int threads, cudaStream_t s, int64_t* blocks_out);
 
 }  // namespace ensd

@@ -36,24 +36,24 @@ ENS_MVS_SHAPE(15, 5, 3, 128, 255)
 ENS_MVS_SHAPE(16, 5, 3, 128, 255)
 #undef ENS_MVS_SHAPE
 
-template <int N>
+template <int N, bool MERGED = false>
 constexpr auto kernel_ptr() {
     using S = MvsShape<N>;
-    return &mvs_kernel<N, S::L, S::B, S::MAXREG>;
+    return &mvs_kernel<N, S::L, S::B, S::MAXREG, MERGED>;
 }
 
-template <int N>
+template <int N, bool MERGED = false>
 KernelInfo info_of() {
     using S = MvsShape<N>;
     KernelInfo k;
-    k.fn = (const void*)kernel_ptr<N>();
+    k.fn = (const void*)kernel_ptr<N, MERGED>();
     k.shape.L = S::L;
     k.shape.B = S::B;
     k.threads = S::THREADS;
     return k;
 }
 
-template <int N>
+template <int N, bool MERGED>
 cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
     using S = MvsShape<N>;
     if (threads > S::THREADS) threads = S::THREADS;  // __launch_bounds__ of the kernel
@@ -62,7 +62,7 @@ cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t
     const int wpb = threads / 32;
     const int64_t blocks = (warps + wpb - 1) / wpb;
     if (blocks_out) *blocks_out = blocks;
-    kernel_ptr<N>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
+    kernel_ptr<N, MERGED>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
     return cudaGetLastError();
 }
 
@@ -70,10 +70,10 @@ cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t
 
 #define ENS_FOR_EACH_N(X) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
 
-KernelInfo mvs_kernel_for(int n_body) {
+KernelInfo mvs_kernel_for(int n_body, bool merged) {
     switch (n_body) {
 #define X(N_) \
-    case N_: return info_of<N_>();
+    case N_: return merged ? info_of<N_, true>() : info_of<N_>();
         ENS_FOR_EACH_N(X)
 #undef X
     }
@@ -84,10 +84,10 @@ KernelInfo mvs_kernel_for(int n_body) {
     return none;
 }
 
-cudaError_t launch_mvs(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
+cudaError_t launch_mvs(const View& v, const StepArgs& a, bool merged, int threads, cudaStream_t s, int64_t* blocks_out) {
     switch (v.n_body) {
 #define X(N_) \
-    case N_: return launch_n<N_>(v, a, threads, s, blocks_out);
+    case N_: return merged ? launch_n<N_, true>(v, a, threads, s, blocks_out) : launch_n<N_, false>(v, a, threads, s, blocks_out);
         ENS_FOR_EACH_N(X)
 #undef X
     }

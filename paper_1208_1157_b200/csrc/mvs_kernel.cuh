@@ -262,7 +262,15 @@ __device__ __forceinline__ void mass_weighted_sum(const double (&W)[B][3], const
 
 // MAXREG caps the registers per thread (and with them the resident warps per SM) directly: __launch_bounds__'s
 // minBlocks lets ptxas round down to a register count that spills.  Blocks must not exceed 65536 / MAXREG threads.
-template <int N, int L, int B, int MAXREG>
+// MERGED = true (ENS_MVS_MERGED): the adjacent half sub-steps of consecutive steps are merged.  The
+// closing half drift of step k and the opening one of step k+1 use the same drift velocity (one full drift), and the
+// kick commutes with the Cartesian drift (the planets' mutual accelerations carry no net momentum, so the drift
+// velocity is the same before and after a kick; the drift moves all planets alike, so A is unchanged): the two
+// half kicks around the merged drift are one full kick.  A step is then  Kepler drift | A | full kick | full drift,
+// opened by half drift + half kick and closed by half kick + half drift when the system leaves the loop.  The
+// post-step positions Alg. 1 shows the monitors are formed as temporaries.  Same map in exact arithmetic; rounding
+// differs from the unmerged kernel and oracle (tests/test_gpu_mvs_merged.py states the distance).
+template <int N, int L, int B, int MAXREG, bool MERGED = false>
 __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
     constexpr int P = N - 1;   // planets; body 0 is the star
     constexpr int S = 32 / L;  // systems per warp
@@ -359,11 +367,8 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
         }
     }
 
-    while (true) {
-        const unsigned amask = __ballot_sync(0xffffffffu, active);
-        if (amask == 0) break;
-        if (active) {
-            // 1 + 2: Cartesian half drift, half kick
+    if constexpr (MERGED) {
+        if (active) {  // open: half drift, half kick
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const double sh = hh * s[c];
@@ -374,26 +379,64 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
                 }
                 Xcm[c] = fma(hh, Vcm[c], Xcm[c]);
             }
+        }
+    }
+    while (true) {
+        const unsigned amask = __ballot_sync(0xffffffffu, active);
+        if (amask == 0) break;
+        if (active) {
+            double Qp[B][3], Xp[3];  // MERGED: post-step positions (after the closing half drift), temporaries
+            if constexpr (!MERGED) {
+                // 1 + 2: Cartesian half drift, half kick
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const double sh = hh * s[c];
+#pragma unroll
+                    for (int b = 0; b < B; ++b) {
+                        Q[b][c] += sh;
+                        V[b][c] = fma(hh, A[b][c], V[b][c]);
+                    }
+                    Xcm[c] = fma(hh, Vcm[c], Xcm[c]);
+                }
+            }
             // 3: Kepler drift of every planet about mu = G m_0 (G = 1)
             kepler_drift_all<B>(Q, V, m0, h, [&](int b) { return !PADDED || (l * B + b < P); });
+            if constexpr (MERGED) {
+                // drift velocity of the rest of this step and the start of the next: kicks do not change it
+                mass_weighted_sum<L, B>(V, m, s, l, base, amask);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) s[c] = s[c] * im0;
+            }
             // 4: planet-planet accelerations at the new positions, half kick
             eval_acc_planets<P, L, B>(Q, m, A, r2min, l, base, amask);
+            if constexpr (!MERGED) {
 #pragma unroll
-            for (int b = 0; b < B; ++b)
+                for (int b = 0; b < B; ++b)
 #pragma unroll
-                for (int c = 0; c < 3; ++c) V[b][c] = fma(hh, A[b][c], V[b][c]);
-            // 5: Cartesian half drift with the new momenta
-            mass_weighted_sum<L, B>(V, m, s, l, base, amask);
+                    for (int c = 0; c < 3; ++c) V[b][c] = fma(hh, A[b][c], V[b][c]);
+                // 5: Cartesian half drift with the new momenta
+                mass_weighted_sum<L, B>(V, m, s, l, base, amask);
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                s[c] = s[c] * im0;
-                const double sh = hh * s[c];
+                for (int c = 0; c < 3; ++c) {
+                    s[c] = s[c] * im0;
+                    const double sh = hh * s[c];
 #pragma unroll
-                for (int b = 0; b < B; ++b) Q[b][c] += sh;
-                Xcm[c] = fma(hh, Vcm[c], Xcm[c]);
+                    for (int b = 0; b < B; ++b) Q[b][c] += sh;
+                    Xcm[c] = fma(hh, Vcm[c], Xcm[c]);
+                }
+            } else {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const double sh = hh * s[c];
+#pragma unroll
+                    for (int b = 0; b < B; ++b) Qp[b][c] = Q[b][c] + sh;
+                    Xp[c] = fma(hh, Vcm[c], Xcm[c]);
+                }
             }
             t += h;
             ++k;
+            const double(&Qm)[B][3] = MERGED ? Qp : Q;  // the post-step positions
+            const double(&Xm)[3] = MERGED ? Xp : Xcm;
 
             // monitors on the post-step state (Alg. 1 execute(M); R11).  Planet-planet separations are
             // those of the acceleration evaluation: the drift shifts every planet alike.
@@ -403,7 +446,7 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
 #pragma unroll
             for (int b = 0; b < B; ++b) {
                 if (!PADDED || (l * B + b < P)) {
-                    const u64 q2 = dbits(fma(Q[b][2], Q[b][2], fma(Q[b][1], Q[b][1], Q[b][0] * Q[b][0])));
+                    const u64 q2 = dbits(fma(Qm[b][2], Qm[b][2], fma(Qm[b][1], Qm[b][1], Qm[b][0] * Qm[b][0])));
                     q2max = q2 > q2max ? q2 : q2max;
                     q2min = q2 < q2min ? q2 : q2min;
                 }
@@ -412,14 +455,14 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
             if (q2min < p.rc2_bits) f |= 1;
             if (mon_eject) {  // distances from the coordinate origin need the star's barycentric position
                 double sq[3], x0[3];
-                mass_weighted_sum<L, B>(Q, m, sq, l, base, amask);
+                mass_weighted_sum<L, B>(Qm, m, sq, l, base, amask);
 #pragma unroll
-                for (int c = 0; c < 3; ++c) x0[c] = Xcm[c] - sq[c] / Mtot;
+                for (int c = 0; c < 3; ++c) x0[c] = Xm[c] - sq[c] / Mtot;
                 if (dbits(fma(x0[2], x0[2], fma(x0[1], x0[1], x0[0] * x0[0]))) > p.re2_bits) f |= 2;
 #pragma unroll
                 for (int b = 0; b < B; ++b) {
                     if (!PADDED || (l * B + b < P)) {
-                        const double xx = x0[0] + Q[b][0], yy = x0[1] + Q[b][1], zz = x0[2] + Q[b][2];
+                        const double xx = x0[0] + Qm[b][0], yy = x0[1] + Qm[b][1], zz = x0[2] + Qm[b][2];
                         if (dbits(fma(zz, zz, fma(yy, yy, xx * xx))) > p.re2_bits) f |= 2;
                     }
                 }
@@ -443,6 +486,29 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
             } else if (k >= p.max_steps) {
                 st = ENS_DONE_STEPS;
                 active = false;
+            }
+            if constexpr (MERGED) {
+                if (active) {  // full kick and full drift: the closing halves of this step and the opening ones of the next
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                        for (int b = 0; b < B; ++b) {
+                            V[b][c] = fma(h, A[b][c], V[b][c]);
+                            Q[b][c] = fma(h, s[c], Q[b][c]);
+                        }
+                        Xcm[c] = fma(h, Vcm[c], Xcm[c]);
+                    }
+                } else {  // the system leaves the loop: close the step
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                        for (int b = 0; b < B; ++b) {
+                            V[b][c] = fma(hh, A[b][c], V[b][c]);
+                            Q[b][c] = Qp[b][c];
+                        }
+                        Xcm[c] = Xp[c];
+                    }
+                }
             }
         }
     }

@@ -36,17 +36,20 @@ ENS_RK_SHAPE(15, 5, 3, 64, 255)
 ENS_RK_SHAPE(16, 5, 4, 64, 255)
 #undef ENS_RK_SHAPE
 
-template <int N>
+template <int N, bool ADAPT = false>
 constexpr auto kernel_ptr() {
     using S = RkShape<N>;
-    return &rkck_kernel<N, S::L, S::B, S::MAXREG>;
+    if constexpr (ADAPT)
+        return &rkck_adaptive_kernel<N, S::L, S::B, S::MAXREG>;
+    else
+        return &rkck_kernel<N, S::L, S::B, S::MAXREG>;
 }
 
-template <int N>
+template <int N, bool ADAPT = false>
 KernelInfo info_of() {
     using S = RkShape<N>;
     KernelInfo k;
-    k.fn = (const void*)kernel_ptr<N>();
+    k.fn = (const void*)kernel_ptr<N, ADAPT>();
     k.shape.L = S::L;
     k.shape.B = S::B;
     k.threads = S::THREADS;
@@ -85,6 +88,62 @@ RkCoef coefficients(double h) {
     return q;
 }
 
+// the same tableau without the powers of h, plus the weights of the embedded error estimate d = b5 - b4 (adaptive kernel)
+RkUnit unit_coefficients() {
+    typedef long double R;
+    const R A[6][5] = {{0, 0, 0, 0, 0},
+                       {R(1) / 5, 0, 0, 0, 0},
+                       {R(3) / 40, R(9) / 40, 0, 0, 0},
+                       {R(3) / 10, R(-9) / 10, R(6) / 5, 0, 0},
+                       {R(-11) / 54, R(5) / 2, R(-70) / 27, R(35) / 27, 0},
+                       {R(1631) / 55296, R(175) / 512, R(575) / 13824, R(44275) / 110592, R(253) / 4096}};
+    const R b5[6] = {R(37) / 378, 0, R(250) / 621, R(125) / 594, 0, R(512) / 1771};
+    const R b4[6] = {R(2825) / 27648, 0, R(18575) / 48384, R(13525) / 55296, R(277) / 14336, R(1) / 4};
+    RkUnit q;
+    for (int i = 0; i < 6; ++i) {
+        R c = 0;
+        for (int j = 0; j < i; ++j) c += A[i][j];
+        q.c[i] = (double)c;
+        q.b[i] = (double)b5[i];
+        q.d[i] = (double)(b5[i] - b4[i]);
+        for (int ll = 0; ll < 4; ++ll) {
+            R s = 0;
+            for (int j = ll + 1; j < i; ++j) s += A[i][j] * A[j][ll];
+            q.AA[i][ll] = (double)s;
+        }
+    }
+    for (int ll = 0; ll < 5; ++ll) {
+        R s = 0, sd = 0;
+        for (int i = ll + 1; i < 6; ++i) {
+            s += b5[i] * A[i][ll];
+            sd += (b5[i] - b4[i]) * A[i][ll];
+        }
+        q.bA[ll] = (double)s;
+        q.dA[ll] = (double)sd;
+    }
+    return q;
+}
+
+template <int N>
+cudaError_t launch_adaptive_n(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
+    using S = RkShape<N>;
+    if (threads > S::THREADS) threads = S::THREADS;
+    const int64_t sys_per_warp = 32 / S::L;
+    const int64_t warps = (v.n_sys + sys_per_warp - 1) / sys_per_warp;
+    const int wpb = threads / 32;
+    int64_t blocks = (warps + wpb - 1) / wpb;
+    int dev = 0, sms = 0, per_sm = 0;  // persistent grid: what the device holds at once
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel_ptr<N, true>(), threads, 0);
+    if (err != cudaSuccess) return err;
+    const int64_t resident = (int64_t)sms * (per_sm > 0 ? per_sm : 1);
+    if (blocks > resident) blocks = resident;
+    if (blocks_out) *blocks_out = blocks;
+    kernel_ptr<N, true>()<<<(unsigned)blocks, threads, 0, s>>>(v, a, unit_coefficients());
+    return cudaGetLastError();
+}
+
 template <int N>
 cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
     using S = RkShape<N>;
@@ -102,10 +161,10 @@ cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t
 
 #define ENS_FOR_EACH_N(X) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15) X(16)
 
-KernelInfo rkck_kernel_for(int n_body) {
+KernelInfo rkck_kernel_for(int n_body, bool adaptive) {
     switch (n_body) {
 #define X(N_) \
-    case N_: return info_of<N_>();
+    case N_: return adaptive ? info_of<N_, true>() : info_of<N_>();
         ENS_FOR_EACH_N(X)
 #undef X
     }
@@ -116,10 +175,10 @@ KernelInfo rkck_kernel_for(int n_body) {
     return none;
 }
 
-cudaError_t launch_rkck(const View& v, const StepArgs& a, int threads, cudaStream_t s, int64_t* blocks_out) {
+cudaError_t launch_rkck(const View& v, const StepArgs& a, bool adaptive, int threads, cudaStream_t s, int64_t* blocks_out) {
     switch (v.n_body) {
 #define X(N_) \
-    case N_: return launch_n<N_>(v, a, threads, s, blocks_out);
+    case N_: return adaptive ? launch_adaptive_n<N_>(v, a, threads, s, blocks_out) : launch_n<N_>(v, a, threads, s, blocks_out);
         ENS_FOR_EACH_N(X)
 #undef X
     }

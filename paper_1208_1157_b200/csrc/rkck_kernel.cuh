@@ -177,4 +177,280 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Adaptive-step Cash-Karp (reading R-RK2' of DESIGN.md section 3: the step-size control the GSL
+// manual documents for the stepper the paper follows, step factors from a discrete set).  Per system and trial step h:
+//   error level  r = max( max|err_x| / (eps X), max|err_v| / (eps V) ),  err = fifth minus fourth order solution,
+//                X = max_b |x_b|, V = max_b |v_b| at the start of the step;
+//   r > 1.1      rejected: state and time untouched, h <- h max(1/5, F(0.9 r^(-1/4))), next trial;
+//   otherwise    accepted; if r < 0.5 the next step starts from h <- h min(5, max(1, F(0.9 r^(-1/5))));  F(f) = floor(16 f) / 16.
+// With k_l the stage accelerations and d = b5 - b4 (sum d_i = 0) the error needs no stage velocities either:
+//   err_x = h^2 sum_l (d A)_l k_l,   err_v = h sum_i d_i k_i.
+// The step size is per system, so the tableau products come without the powers of h (RkUnit, constant bank) and h, h^2
+// multiply the sums.  Stage 1 depends on the positions only: a rejected trial keeps it (bit-identical to re-evaluating).
+// Systems take different numbers of trials, so the grid is persistent and every group of L lanes pulls the next system
+// from a device counter when its own is finished (as the adaptive Hermite kernel does).
+// ---------------------------------------------------------------------------------------------------------------
+struct RkUnit {
+    double c[6];       // c_i
+    double AA[6][4];   // (A A)_il
+    double bA[5];      // (b5 A)_l
+    double b[6];       // b5_i
+    double dA[5];      // ((b5 - b4) A)_l
+    double d[6];       // b5_i - b4_i
+};
+
+// r^(-1/5) for 1e-4 <= r < 0.5: FP32 seed (exp2 / log2 approximations, ~1e-6) and two Newton steps for y^-5 = r
+__device__ __forceinline__ double inv_fifth_root(double r) {
+    double y = (double)exp2f(-0.2f * __log2f((float)r));
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const double y2 = y * y, y5 = (y2 * y2) * y;
+        y = fma(0.2 * y, fma(-r, y5, 1.0), y);
+    }
+    return y;
+}
+
+template <int N, int L, int B, int MAXREG>
+__global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkUnit q) {
+    constexpr int S = 32 / L;
+    constexpr bool PADDED = (L * B != N);
+    const int lane = threadIdx.x & 31;
+    const int sl = lane / L;
+    const int l = lane - sl * L;
+    const int base = sl * L;
+    int64_t sys = 0;
+
+    double X[B][3], V[B][3], m[B];
+    double t = 0.0, h = p.dt;
+    int st = ENS_STOP_NONFINITE;
+    bool active = false, writeback = false, have_k1 = false;
+    int64_t k = 0, nrej = 0;
+    bool exhausted = !(sl < S);
+    const bool fwd = p.dt > 0.0;
+    const double ieps = 1.0 / p.rk_eps;
+
+    auto load_system = [&]() {
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const int gid = l * B + b;
+            X[b][0] = 1.0e8 * (double)(gid + 1);  // dummy slot (padded shapes): massless, far from everything
+            X[b][1] = X[b][2] = 0.0;
+            V[b][0] = V[b][1] = V[b][2] = 0.0;
+            m[b] = 0.0;
+            if (!PADDED || gid < N) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    X[b][c] = e.pos[(int64_t)(gid * 3 + c) * e.n_pad + sys];
+                    V[b][c] = e.vel[(int64_t)(gid * 3 + c) * e.n_pad + sys];
+                }
+                m[b] = e.mass[(int64_t)gid * e.n_pad + sys];
+            }
+        }
+        t = e.time[sys];
+        st = e.status[sys];
+        k = nrej = 0;
+        h = p.dt;  // every call starts every system from the caller's trial step
+        have_k1 = false;
+        active = st < ENS_STOP_CLOSE;
+        writeback = active;
+    };
+    auto store_system = [&]() {
+        if (writeback) {
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                const int gid = l * B + b;
+                if (!PADDED || gid < N) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        e.pos[(int64_t)(gid * 3 + c) * e.n_pad + sys] = X[b][c];
+                        e.vel[(int64_t)(gid * 3 + c) * e.n_pad + sys] = V[b][c];
+                    }
+                }
+            }
+            if (l == 0) {
+                e.time[sys] = t;
+                e.status[sys] = st;
+                e.nsteps[sys] += k;
+                e.nreject[sys] += nrej;
+            }
+        }
+        writeback = false;
+    };
+    auto refill = [&]() -> bool {  // whole warp converged
+        const bool want = !active && !exhausted;
+        const unsigned rmask = __ballot_sync(0xffffffffu, want);
+        if (want) {
+            store_system();
+            unsigned long long idx = 0;
+            if (l == 0) idx = atomicAdd(p.counter, 1ull);
+            if constexpr (L > 1) idx = __shfl_sync(rmask, idx, base);
+            if ((int64_t)idx < e.n_sys) {
+                sys = (int64_t)idx;
+                load_system();
+            } else {
+                exhausted = true;
+            }
+        }
+        return __ballot_sync(0xffffffffu, !exhausted) != 0;
+    };
+    // maximum over the L lanes of a system (all lanes of `mask` systems take part)
+    auto lanes_max = [&](double v, unsigned mask) {
+        if constexpr (L > 1) {
+            double g = v;
+#pragma unroll
+            for (int i = 1; i < L; ++i) {
+                int li = l + i;
+                if (li >= L) li -= L;
+                g = fmax(g, __shfl_sync(mask, v, base + li));
+            }
+            return g;
+        } else {
+            return v;
+        }
+    };
+
+    double K[5][B][3];  // stage accelerations k_1 .. k_5
+    u64 r2min;
+
+    while (true) {
+        if (!refill()) break;
+        const unsigned amask = __ballot_sync(0xffffffffu, active);
+        if (amask == 0) continue;
+        if (active) {
+            // stage 1 at the accepted state (after an accepted step or at the start of the run): also the monitors'
+            // pair distances (Alg. 1: advance, then execute(M)) and the loop tests.  A rejected trial skips all this.
+            const unsigned kmask = (L > 1) ? __ballot_sync(amask, !have_k1) : amask;
+            if (!have_k1) {
+                eval_acc_planets<N, L, B>(X, m, K[0], r2min, l, base, kmask);
+                have_k1 = true;
+                int f = (r2min < p.rc2_bits) ? 1 : 0;
+#pragma unroll
+                for (int b = 0; b < B; ++b) {
+                    const u64 db = dbits(fma(X[b][2], X[b][2], fma(X[b][1], X[b][1], X[b][0] * X[b][0])));
+                    if (!PADDED || (l * B + b < N)) {
+                        if (db > p.re2_bits) f |= 2;
+                        if (db > 0x7FEFFFFFFFFFFFFFull) f |= 4;
+                    }
+                }
+                if constexpr (L > 1) {
+                    int g = f;
+#pragma unroll
+                    for (int i = 1; i < L; ++i) {
+                        int li = l + i;
+                        if (li >= L) li -= L;
+                        g |= __shfl_sync(kmask, f, base + li);
+                    }
+                    f = g;
+                }
+                if (k > 0 && f) {
+                    st = (f & 4) ? ENS_STOP_NONFINITE : (f & 1) ? ENS_STOP_CLOSE : ENS_STOP_EJECT;
+                    active = false;
+                } else if (!(fwd ? (t < p.t_end) : (t > p.t_end))) {
+                    st = ENS_DONE_TIME;
+                    active = false;
+                } else if (k >= p.max_steps) {
+                    st = ENS_DONE_STEPS;
+                    active = false;
+                }
+            }
+            unsigned am2 = amask;
+            if constexpr (L > 1) am2 = __ballot_sync(amask, active);
+            if (active) {
+                const double h2 = h * h;
+                double Xs[B][3], K6[B][3];
+                u64 dummy;
+#pragma unroll
+                for (int i = 1; i < 6; ++i) {  // stages 2 .. 6
+                    const double ch = q.c[i] * h;
+#pragma unroll
+                    for (int b = 0; b < B; ++b)
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            double s = 0.0;
+#pragma unroll
+                            for (int ll = 0; ll + 2 <= i; ++ll) s = fma(q.AA[i][ll], K[ll][b][c], s);
+                            Xs[b][c] = fma(h2, s, fma(ch, V[b][c], X[b][c]));
+                        }
+                    if (i < 5)
+                        eval_acc_planets<N, L, B>(Xs, m, K[i], dummy, l, base, am2);
+                    else
+                        eval_acc_planets<N, L, B>(Xs, m, K6, dummy, l, base, am2);
+                }
+                // error level of this trial (scales from the state the step starts from)
+                double ex = 0.0, ev = 0.0, x2 = 0.0, v2 = 0.0;
+#pragma unroll
+                for (int b = 0; b < B; ++b) {
+                    if (!PADDED || (l * B + b < N)) {
+                        x2 = fmax(x2, fma(X[b][2], X[b][2], fma(X[b][1], X[b][1], X[b][0] * X[b][0])));
+                        v2 = fmax(v2, fma(V[b][2], V[b][2], fma(V[b][1], V[b][1], V[b][0] * V[b][0])));
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            double sx = 0.0;
+#pragma unroll
+                            for (int ll = 0; ll < 5; ++ll) sx = fma(q.dA[ll], K[ll][b][c], sx);
+                            double sv = q.d[0] * K[0][b][c];  // d_2 = 0
+                            sv = fma(q.d[2], K[2][b][c], sv);
+                            sv = fma(q.d[3], K[3][b][c], sv);
+                            sv = fma(q.d[4], K[4][b][c], sv);
+                            sv = fma(q.d[5], K6[b][c], sv);
+                            ex = fmax(ex, fabs(sx));
+                            ev = fmax(ev, fabs(sv));
+                        }
+                    }
+                }
+                ex = lanes_max(ex, am2) * h2;
+                ev = lanes_max(ev, am2) * fabs(h);
+                x2 = lanes_max(x2, am2);
+                v2 = lanes_max(v2, am2);
+                // r = max(ex / (eps |x|), ev / (eps |v|)); NaN (a broken state) compares false everywhere: accepted, and
+                // the non-finite monitor stops the system at its next stage 1
+                const double rx = (ex * ieps) * rsqrt_f64(x2), rv = (ev * ieps) * rsqrt_f64(v2);
+                const double r = rx > rv ? rx : rv;
+                if (r > 1.1) {
+                    double f = 0.2;
+                    if (r < 1e300) {
+                        const double g = rsqrt_f64(r * rsqrt_f64(r));  // r^(-1/4)
+                        f = floor(16.0 * (0.9 * g)) * 0.0625;
+                        if (!(f >= 0.2)) f = 0.2;
+                    }
+                    h *= f;
+                    ++nrej;
+                    if (t + h == t) {  // the step no longer advances the time
+                        st = ENS_STOP_STEPSIZE;
+                        active = false;
+                    }
+                } else {
+#pragma unroll
+                    for (int b = 0; b < B; ++b)
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            double s = 0.0;
+#pragma unroll
+                            for (int ll = 0; ll < 5; ++ll) s = fma(q.bA[ll], K[ll][b][c], s);
+                            X[b][c] = fma(h2, s, fma(h, V[b][c], X[b][c]));
+                            double w = q.b[0] * K[0][b][c];  // b_2 = b_5 = 0
+                            w = fma(q.b[2], K[2][b][c], w);
+                            w = fma(q.b[3], K[3][b][c], w);
+                            w = fma(q.b[5], K6[b][c], w);
+                            V[b][c] = fma(h, w, V[b][c]);
+                        }
+                    t += h;
+                    ++k;
+                    have_k1 = false;
+                    if (r < 0.5) {
+                        double f = 5.0;
+                        if (r >= 1e-4) {
+                            f = floor(16.0 * (0.9 * inv_fifth_root(r))) * 0.0625;
+                            f = f > 5.0 ? 5.0 : f < 1.0 ? 1.0 : f;
+                        }
+                        h *= f;
+                    }
+                }
+            }
+        }
+    }
+    store_system();
+}
+
 }  // namespace ensd

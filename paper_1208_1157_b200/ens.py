@@ -13,9 +13,10 @@ import numpy as np
 import torch
 
 OK, EINVAL, ENOMEM, ECUDA, ESTATE, EUNSUPPORTED = 0, -1, -2, -3, -4, -5
-HERMITE, MVS, HERMITE_ADAPTIVE, HERMITE_CARRY, RKCK = 0, 1, 2, 3, 4  # HERMITE_ADAPTIVE: `dt` is the step size scale tau of Eq. 5
+# HERMITE_ADAPTIVE: `dt` is the step size scale tau of Eq. 5; RKCK_ADAPTIVE: `dt` is the first trial step
+HERMITE, MVS, HERMITE_ADAPTIVE, HERMITE_CARRY, RKCK, MVS_MERGED, RKCK_ADAPTIVE = 0, 1, 2, 3, 4, 5, 6
 HOST, DEVICE = 0, 1
-ACTIVE, DONE_TIME, DONE_STEPS, STOP_CLOSE, STOP_EJECT, STOP_NONFINITE = range(6)
+ACTIVE, DONE_TIME, DONE_STEPS, STOP_CLOSE, STOP_EJECT, STOP_NONFINITE, STOP_STEPSIZE = range(7)
 LOG_SNAPSHOTS, LOG_STOPS = 1, 2
 OPT_THREADS, OPT_ADAPTIVE_UNORDERED, OPT_SLICE_MODE, OPT_SLICE_STEPS, OPT_SLICE_WARPS_PER_SM = range(5)
 
@@ -26,7 +27,7 @@ SYMBOLS = (
     "ens_create", "ens_destroy", "ens_set_state", "ens_set_monitors", "ens_integrate", "ens_get_state",
     "ens_energy", "ens_strerror", "ens_get_info", "ens_last_kernel_ms", "ens_fp64_peak", "ens_test_rsqrt",
     "ens_test_rcp", "ens_log_enable", "ens_integrate_logged", "ens_log_read", "ens_reserve_host_staging",
-    "ens_test_set_option",
+    "ens_test_set_option", "ens_set_rk_tolerance", "ens_get_rejected",
 )
 _lib = None
 
@@ -72,6 +73,8 @@ def lib() -> ctypes.CDLL:
         L.ens_log_enable.argtypes = [vp, i64, vp]
         L.ens_integrate_logged.argtypes = [vp, ci, cd, cd, i64, i64, ci, vp]
         L.ens_reserve_host_staging.argtypes = [vp]
+        L.ens_set_rk_tolerance.argtypes = [vp, cd]
+        L.ens_get_rejected.argtypes = [vp, vp, ci, vp]
         L.ens_test_set_option.argtypes = [vp, ci, i64]
         L.ens_log_read.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64), vp, vp, vp, vp, vp, vp, i64, ci, vp]
         for name in SYMBOLS:
@@ -154,6 +157,15 @@ class Ensemble:
     # -- ens_set_monitors ---------------------------------------------------------------------------
     def set_monitors(self, r_close: float = 0.0, r_eject: float = float("inf")):
         _check(lib().ens_set_monitors(self._h, float(r_close), float(r_eject)), "ens_set_monitors")
+
+    # -- ens_set_rk_tolerance / ens_get_rejected -------------------------------------------------------
+    def set_rk_tolerance(self, eps: float):
+        _check(lib().ens_set_rk_tolerance(self._h, float(eps)), "ens_set_rk_tolerance")
+
+    def get_rejected(self, stream=None):
+        out = np.empty(self.n_sys, np.int64)
+        _check(lib().ens_get_rejected(self._h, out.ctypes.data, HOST, _stream_ptr(stream)), "ens_get_rejected")
+        return out
 
     # -- ens_integrate ------------------------------------------------------------------------------
     def integrate(self, integrator: int, dt: float, max_steps: int, t_end: float = float("inf"), stream=None):
@@ -264,15 +276,18 @@ def rcp_probe(x: torch.Tensor) -> torch.Tensor:
 
 
 def run(cfg_or_integrator, pos, vel, mass, *, dt, steps, r_close=0.0, r_eject=float("inf"), t_end=float("inf"),
-        time=None, want_energy=False):
+        time=None, want_energy=False, rk_eps=None):
     """Convenience: create, set, integrate, get (host arrays in, host arrays out).  Used by the tests."""
     n_sys, n_body = mass.shape
     with Ensemble(n_sys, n_body) as e:
         e.set_state(pos, vel, mass, time)
         e.set_monitors(r_close, r_eject)
+        if rk_eps is not None:
+            e.set_rk_tolerance(rk_eps)
         E0 = e.energy() if want_energy else None
         e.integrate(cfg_or_integrator, dt, steps, t_end)
         out = e.get_state()
+        out["nreject"] = e.get_rejected()
         if want_energy:
             out["E0"], out["L0"] = E0
             out["E"], out["L"] = e.energy()

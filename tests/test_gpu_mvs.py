@@ -97,8 +97,12 @@ def test_large_steps_eccentric_and_negative_dt():
             d, floor = rel_diff(g[key], o[key]), rel_diff(o[key], ol[key])
             # steps this coarse make some systems chaotic: judge the ensemble median and each system against the
             # oracle's own double-vs-long-double rounding floor (R-noise), never against a fixed number
+            ratio = d / np.maximum(1e-11, floor)
+            print(f"large steps dt={dt} {key}: gpu-vs-oracle median {np.median(d):.2e} max {d.max():.2e}; floor median "
+                  f"{np.median(floor):.2e} max {floor.max():.2e}; worst d / max(1e-11, floor) = {ratio.max():.2f}; "
+                  f"systems beyond max(1e-10, 10 floor): {(d > np.maximum(1e-10, 10 * floor)).sum()} of {len(d)}")
             assert np.median(d) <= 3 * np.median(floor) + 1e-13, (key, dt, np.median(d), np.median(floor))
-            assert (d <= np.maximum(1e-10, 30 * floor)).all(), (key, dt, (d / np.maximum(1e-11, floor)).max())
+            assert (d <= np.maximum(1e-10, 10 * floor)).all(), (key, dt, ratio.max())  # R-noise (ii): 10 x
     with ens.Ensemble(160, 4) as e:
         e.set_state(pos, vel, mass)
         e.integrate(ens.MVS, 0.05, 400)
@@ -111,7 +115,11 @@ def test_large_steps_eccentric_and_negative_dt():
     of = oracle.integrate(oracle.MVS, pos, vel, mass, dt=0.05, max_steps=400)
     orv = oracle.integrate(oracle.MVS, of["pos"], of["vel"], mass, of["time"], dt=-0.05, max_steps=400, t_end=-np.inf)
     d, dref = rel_diff(r["pos"], pos), rel_diff(orv["pos"], pos)
+    print(f"reversal defect: gpu median {np.median(d):.2e} max {d.max():.2e}; oracle's own median {np.median(dref):.2e} "
+          f"max {dref.max():.2e}; systems where the ORACLE's defect exceeds 1e-10: {(dref > 1e-10).sum()}, the gpu's: "
+          f"{(d > 1e-10).sum()}; worst d / max(1e-11, oracle's) = {(d / np.maximum(1e-11, dref)).max():.2f}")
     assert (d <= np.maximum(1e-11, 10 * dref)).all(), (d / np.maximum(1e-11, dref)).max()
+    assert d.max() <= 1e-10  # the absolute bar of the round-1 test, met again (measured 8.2e-11; the oracle's own: 4.6e-11)
     assert np.median(d) <= 1e-12 and np.abs(r["time"]).max() <= 1e-12
 
 
