@@ -9,7 +9,7 @@ import torch
 import oracle
 from paper_1208_1157_b200 import ens
 from paper_1208_1157_b200 import workloads as W
-from parity import energy_err, rel_diff, run_cuda, run_oracle
+from parity import energy_err, knife_edge_systems, rel_diff, run_cuda, run_oracle
 
 pytestmark = pytest.mark.gpu
 
@@ -44,9 +44,16 @@ def test_full_size_launch_sampled_parity(cfg, n_sample):
     idx = np.unique(np.concatenate([strided, stopped]))
     o = run_oracle(c, pos[idx], vel[idx], mass[idx])
     ol = run_oracle(c, pos[idx], vel[idx], mass[idx], prec=oracle.LONG_DOUBLE)
-    # knife-edge exemption (R12): a stop decided within 1e-9 relative of the threshold may differ by a step
+    # R12 as written: (status, stop step) exact; a mismatch is allowed only where the oracle's deciding separation /
+    # radius is within 1e-9 (relative) of the threshold, which is checked system by system (count reported)
     same = (g["status"][idx] == o["status"]) & (g["nsteps"][idx] == o["nsteps"])
-    assert same.mean() >= 0.99, f"status/nsteps mismatches: {(~same).sum()} of {len(idx)}"
+    n_edge = knife_edge_systems(c, pos[idx], vel[idx], mass[idx], g["status"][idx], g["nsteps"][idx], o["status"], o["nsteps"])
+    print(f"cfg{cfg}: {n_edge} knife-edge system(s) of {len(idx)} sampled (stops among them: {(o['status'] >= oracle.STOP_CLOSE).sum()})")
+    # a stopped system keeps its post-step state: compared like any other state
+    stopped = same & (o["status"] >= oracle.STOP_CLOSE)
+    if stopped.any():
+        assert rel_diff(g["pos"][idx][stopped], o["pos"][stopped]).max() <= 1e-6
+        assert (g["time"][idx][stopped] == o["time"][stopped]).all()
     ok = same & (o["status"] == oracle.DONE_STEPS) & (ol["status"] == oracle.DONE_STEPS)
     # "stable, well separated" made operational: oracle double and long double agree to 1e-8
     floor_p = rel_diff(o["pos"], ol["pos"])
@@ -211,6 +218,33 @@ def test_monitors_stop_step_and_state_match_oracle():
     assert (g["time"] == o["time"]).all()
     # a stopped system keeps its post-step state
     assert rel_diff(g["pos"], o["pos"]).max() <= 1e-9 and rel_diff(g["vel"], o["vel"]).max() <= 1e-9
+
+
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_monitors_stop_state_matches_oracle_many_lane_shapes(cfg):
+    """The same hand-built stops at n_body = 6 (one system per thread, 15 pairs per lane) and n_body = 15 (5 lanes x 3
+    bodies: shuffled minimum and flag reduction): status, stop step, time exact; the stop STATE compared too."""
+    c = W.CONFIGS[cfg]
+    n_sys, nb = 120, c.n_body
+    pos, vel, mass = W.generate(cfg, n_sys=n_sys)
+    for s in range(n_sys):
+        k = 1 + s % (nb - 2)  # the planet the last body is aimed at / which lane it lives on varies
+        if s % 2 == 1:
+            d = np.array([0.05 + 0.0007 * s, 0.003, 0.001])
+            pos[s, nb - 1] = pos[s, k] + d
+            vel[s, nb - 1] = vel[s, k] - d / np.linalg.norm(d) * (0.4 + 0.01 * (s % 7))
+        elif s % 4 == 0:
+            pos[s, nb - 1] = np.array([6.0, 0.0, 0.0])
+            vel[s, nb - 1] = np.array([2.5 + 0.05 * (s % 5), 0.3, 0.0])
+    kw = dict(dt=0.002, r_close=0.02, r_eject=9.0)
+    g = ens.run(ens.HERMITE, pos, vel, mass, steps=2500, **kw)
+    o = oracle.integrate(oracle.HERMITE, pos, vel, mass, max_steps=2500, **kw)
+    assert (o["status"] == oracle.STOP_CLOSE).sum() >= 40 and (o["status"] == oracle.STOP_EJECT).sum() >= 20
+    assert (g["status"] == o["status"]).all() and (g["nsteps"] == o["nsteps"]).all() and (g["time"] == o["time"]).all()
+    stopped = o["status"] >= oracle.STOP_CLOSE
+    assert rel_diff(g["pos"][stopped], o["pos"][stopped]).max() <= 1e-9
+    assert rel_diff(g["vel"][stopped], o["vel"][stopped]).max() <= 1e-9
+    assert rel_diff(g["pos"], o["pos"]).max() <= 1e-9
 
 
 def test_stop_is_sticky_until_set_state():
