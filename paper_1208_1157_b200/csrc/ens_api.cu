@@ -554,8 +554,7 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
     a.order = nullptr;
     a.slice_done = e->slice_done;
     a.rk_eps = e->rk_eps;
-    if (integrator == ENS_RKCK_ADAPTIVE) CU(cudaMemsetAsync(e->counter, 0, sizeof(unsigned long long), s));
-    if (integrator == ENS_HERMITE_ADAPTIVE) {
+    if (integrator == ENS_HERMITE_ADAPTIVE || integrator == ENS_RKCK_ADAPTIVE) {
         CU(cudaMemsetAsync(e->counter, 0, sizeof(unsigned long long), s));
         if (!e->tune.adaptive_unordered && e->order.idx_out) {
             CU(ensd::adaptive_order(e->v, t_end, e->order, s));

@@ -13,17 +13,11 @@ __device__ __forceinline__ u64 dbits(double x) { return (u64)__double_as_longlon
 // cubic Newton-Halley step in FP64,
 //   e = 1 - r2 y0^2,  y = y0 + y0 e (1/2 + 3/8 e),   remaining error ~ (5/16) e^3 < 2^-61 plus rounding: <= 1 ulp
 // (tests/test_gpu_hermite.py::test_rsqrt_within_one_ulp measures it).  Valid for normal, finite r2 > 0.
-// -DENS_SEED_F32 selects the older seed (FP32 MUFU.RSQ of the value rounded to float: two extra F2F per call, and
-// r2 restricted to the FP32 range); it was 2-6 % slower in every kernel.
+// (An FP32 seed - MUFU.RSQ of the value rounded to float, two extra F2F per call, r2 restricted to the FP32 range - was
+// 2-6 % slower in every kernel: DESIGN.md section 8.)
 __device__ __forceinline__ double rsqrt_f64(double r2) {
     double y0;
-#ifndef ENS_SEED_F32
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(r2));
-#else
-    float s;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(__double2float_rn(r2)));
-    y0 = (double)s;
-#endif
     const double t = r2 * y0;
     const double e = fma(-t, y0, 1.0);
     const double p = fma(0.375, e, 0.5);
@@ -37,14 +31,8 @@ __device__ __forceinline__ double rsqrt_f64(double r2) {
 // Valid for normal, finite x != 0.
 template <bool REFINE>
 __device__ __forceinline__ double rcp_f64(double x) {
-#ifndef ENS_SEED_F32
     double y0;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
-#else
-    float s;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(__double2float_rn(x)));
-    const double y0 = (double)s;
-#endif
     const double e = fma(-x, y0, 1.0);
     const double q = y0 * e;
     if constexpr (REFINE) return fma(q, 1.0 + e, y0);

@@ -12,11 +12,20 @@ namespace {
 // recorded in DESIGN.md section 8 (tuning record).
 //   UNROLL   three inlined copies of the evaluation (straight-line step) instead of a 3-phase loop around one copy
 //   THREADS  threads per block;  MAXT, MINB = __launch_bounds__ (register cap 65536 / (MAXT * MINB))
-template <int N> struct ShapeOf;
+//   MODE     0 = fixed step (3 evaluations), 1 = adaptive step, 2 = carried a, j (2 evaluations), 3 = MODE 0 time-sliced
+template <int N> struct ShapeBase;
 #define ENS_SHAPE(N_, L_, B_, UNROLL_, THREADS_, MINB_, MAXT_)                              \
-    template <> struct ShapeOf<N_> {                                                        \
+    template <> struct ShapeBase<N_> {                                                      \
         static constexpr int L = L_, B = B_, THREADS = THREADS_, MINB = MINB_, MAXT = MAXT_; \
         static constexpr bool UNROLL = UNROLL_;                                             \
+    };
+// the shape of (N, MODE): the per-N entry unless a mode has its own launch bounds below (L and B never differ by mode)
+template <int N, int MODE> struct ShapeOf : ShapeBase<N> {};
+#define ENS_SHAPE_MODE(N_, MODE_, UNROLL_, THREADS_, MINB_, MAXT_)                                       \
+    template <> struct ShapeOf<N_, MODE_> {                                                              \
+        static constexpr int L = ShapeBase<N_>::L, B = ShapeBase<N_>::B, THREADS = THREADS_, MINB = MINB_, \
+                             MAXT = MAXT_;                                                               \
+        static constexpr bool UNROLL = UNROLL_;                                                          \
     };
 //        N  L  B  unroll threads minBlocks maxThreads
 ENS_SHAPE(2, 1, 2, true, 64, 1, 128)
@@ -38,19 +47,24 @@ ENS_SHAPE(13, 5, 3, false, 64, 1, 128)
 ENS_SHAPE(14, 5, 3, false, 64, 1, 128)
 ENS_SHAPE(15, 5, 3, false, 64, 1, 128)
 ENS_SHAPE(16, 5, 4, false, 64, 1, 128)
+// the carried accelerations and jerks are 18 more live doubles at n_body = 3: 128 registers spilled 120 B of them
+ENS_SHAPE_MODE(3, 2, true, 64, 5, 64)
+// n_body = 6 with carried a, j: the straight-line step spilled 464 B; the 3-phase loop spills 16 B and is 3.7 % faster
+ENS_SHAPE_MODE(6, 2, false, 32, 1, 32)
 #undef ENS_SHAPE
+#undef ENS_SHAPE_MODE
 
 // MODE: 0 = fixed step (3 evaluations), 1 = adaptive step, 2 = fixed step with carried a, j (2 evaluations),
 //       3 = MODE 0 on a time-sliced persistent grid (same arithmetic, bit-identical results)
 template <int N, int MODE>
 constexpr auto kernel_ptr() {
-    using S = ShapeOf<N>;
+    using S = ShapeOf<N, MODE>;
     return &hermite_kernel<N, S::L, S::B, S::UNROLL, S::MAXT, S::MINB, MODE == 1, MODE == 2, MODE == 3>;
 }
 
 template <int N, int MODE>
 KernelInfo info_of() {
-    using S = ShapeOf<N>;
+    using S = ShapeOf<N, MODE>;
     KernelInfo k;
     k.fn = (const void*)kernel_ptr<N, MODE>();
     k.shape.L = S::L;
@@ -73,7 +87,7 @@ cudaError_t resident_blocks(int threads, int64_t* out) {
 template <int N, int MODE>
 cudaError_t launch_n(const View& v, StepArgs a, const LaunchTune& tune, cudaStream_t s, int64_t* blocks_out,
                      const void** fn_out) {
-    using S = ShapeOf<N>;
+    using S = ShapeOf<N, MODE>;
     int threads = tune.threads ? tune.threads : S::THREADS;
     if (threads > S::MAXT) threads = S::MAXT;  // __launch_bounds__ of the kernel
     const int64_t sys_per_warp = 32 / S::L;
@@ -163,7 +177,7 @@ cudaError_t launch_hermite(const View& v, const StepArgs& a, int mode, const Lau
 int64_t hermite_slice_groups(int64_t n_sys, int n_body) {
     switch (n_body) {
 #define X(N_) \
-    case N_: return (n_sys + 32 / ShapeOf<N_>::L - 1) / (32 / ShapeOf<N_>::L);
+    case N_: return (n_sys + 32 / ShapeBase<N_>::L - 1) / (32 / ShapeBase<N_>::L);
         ENS_FOR_EACH_N(X)
 #undef X
     }

@@ -14,14 +14,8 @@ template <int N> struct MvsShape;
 //            N   L  B  threads maxRegisters
 ENS_MVS_SHAPE(2, 1, 1, 128, 255)
 ENS_MVS_SHAPE(3, 1, 2, 128, 255)
-// config 4 (3 planets): tuned in DESIGN.md §8
-#ifndef ENS_M4_THREADS
-#define ENS_M4_THREADS 64
-#endif
-#ifndef ENS_M4_MAXREG
-#define ENS_M4_MAXREG 168
-#endif
-ENS_MVS_SHAPE(4, 1, 3, ENS_M4_THREADS, ENS_M4_MAXREG)
+// config 4 (3 planets): 64-thread blocks, 168 registers (12 warps per SM): sweeps in DESIGN.md section 8
+ENS_MVS_SHAPE(4, 1, 3, 64, 168)
 ENS_MVS_SHAPE(5, 1, 4, 128, 255)
 ENS_MVS_SHAPE(6, 1, 5, 128, 255)
 ENS_MVS_SHAPE(7, 3, 2, 128, 255)

@@ -192,13 +192,10 @@ __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[
     };
     // Two evaluations are always needed (the second confirms convergence, and is harmless if the first already
     // had): straight-line code for them, a loop only for the rare third and later ones.
-#ifndef ENS_MVS_PEEL
-#define ENS_MVS_PEEL 2
-#endif
     bool done = false;
 #pragma unroll
-    for (int it = 0; it < ENS_MVS_PEEL; ++it) done = iterate();
-    for (int it = ENS_MVS_PEEL; it < 50 && !done; ++it) done = iterate();
+    for (int it = 0; it < 2; ++it) done = iterate();
+    for (int it = 2; it < 50 && !done; ++it) done = iterate();
     if (!done) {  // some planet of this lane did not converge within the cap (or went non-finite): bisect those
 #pragma unroll
         for (int b = 0; b < B; ++b) {

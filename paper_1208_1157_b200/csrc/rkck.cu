@@ -8,19 +8,16 @@ namespace {
 // n_body -> lanes per system L (odd), bodies per lane B, L * B >= n_body.  Five stage accelerations per body live in
 // registers, so a lane holds fewer bodies than in the Hermite kernel.
 template <int N> struct RkShape;
-#define ENS_RK_SHAPE(N_, L_, B_, THREADS_, MAXREG_)                                \
-    template <> struct RkShape<N_> {                                               \
-        static constexpr int L = L_, B = B_, THREADS = THREADS_, MAXREG = MAXREG_; \
+// MAXREG_A: register cap of the adaptive kernel (per-system step size, error sums and counters are live on top)
+#define ENS_RK_SHAPE_A(N_, L_, B_, THREADS_, MAXREG_, MAXREG_A_)                                         \
+    template <> struct RkShape<N_> {                                                                     \
+        static constexpr int L = L_, B = B_, THREADS = THREADS_, MAXREG = MAXREG_, MAXREG_A = MAXREG_A_; \
     };
-#ifndef ENS_RK3_THREADS
-#define ENS_RK3_THREADS 64
-#endif
-#ifndef ENS_RK3_MAXREG
-#define ENS_RK3_MAXREG 168
-#endif
+#define ENS_RK_SHAPE(N_, L_, B_, THREADS_, MAXREG_) ENS_RK_SHAPE_A(N_, L_, B_, THREADS_, MAXREG_, MAXREG_)
 //           N   L  B  threads maxRegisters
 ENS_RK_SHAPE(2, 1, 2, 64, 255)
-ENS_RK_SHAPE(3, 1, 3, ENS_RK3_THREADS, ENS_RK3_MAXREG)
+// n_body = 3 (config 1's ensemble): 168 registers -> 6 blocks of 2 warps per SM, no spills (fixed step)
+ENS_RK_SHAPE_A(3, 1, 3, 64, 168, 232)
 ENS_RK_SHAPE(4, 1, 4, 64, 255)
 ENS_RK_SHAPE(5, 3, 2, 64, 255)
 ENS_RK_SHAPE(6, 3, 2, 64, 255)
@@ -35,12 +32,13 @@ ENS_RK_SHAPE(14, 5, 3, 64, 255)
 ENS_RK_SHAPE(15, 5, 3, 64, 255)
 ENS_RK_SHAPE(16, 5, 4, 64, 255)
 #undef ENS_RK_SHAPE
+#undef ENS_RK_SHAPE_A
 
 template <int N, bool ADAPT = false>
 constexpr auto kernel_ptr() {
     using S = RkShape<N>;
     if constexpr (ADAPT)
-        return &rkck_adaptive_kernel<N, S::L, S::B, S::MAXREG>;
+        return &rkck_adaptive_kernel<N, S::L, S::B, S::MAXREG_A>;
     else
         return &rkck_kernel<N, S::L, S::B, S::MAXREG>;
 }

@@ -286,7 +286,7 @@ __global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkU
             if (l == 0) idx = atomicAdd(p.counter, 1ull);
             if constexpr (L > 1) idx = __shfl_sync(rmask, idx, base);
             if ((int64_t)idx < e.n_sys) {
-                sys = (int64_t)idx;
+                sys = p.order ? (int64_t)p.order[idx] : (int64_t)idx;  // longest expected run first (adaptive_order.cu)
                 load_system();
             } else {
                 exhausted = true;

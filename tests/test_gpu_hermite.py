@@ -334,7 +334,7 @@ def test_error_codes():
     assert L.ens_set_state(h, pos.ctypes.data, vel.ctypes.data, mass.ctypes.data, None, ens.HOST, None) == ens.OK
     for bad_dt in (0.0, float("nan"), float("inf")):
         assert L.ens_integrate(h, ens.HERMITE, bad_dt, float("inf"), 10, None) == ens.EINVAL
-    assert L.ens_integrate(h, 5, 0.01, float("inf"), 10, None) == ens.EINVAL  # 0..4 are the integrators
+    assert L.ens_integrate(h, 7, 0.01, float("inf"), 10, None) == ens.EINVAL  # 0..6 are the integrators
     assert L.ens_integrate(h, -1, 0.01, float("inf"), 10, None) == ens.EINVAL
     assert L.ens_integrate(h, ens.HERMITE, 0.01, float("nan"), 10, None) == ens.EINVAL
     assert L.ens_integrate(h, ens.HERMITE, 0.01, float("inf"), -1, None) == ens.EINVAL
