@@ -123,6 +123,9 @@ __device__ __noinline__ double kepler_bisect(double r0, double eta, double mu, d
 __device__ __forceinline__ int abs_hi(double x) { return __double2hiint(x) & 0x7fffffff; }
 constexpr int kHi0p1 = 0x3fb99999;  // high word of 0.1 (0x3FB999999999999A), rounded down
 constexpr int kHiInf = 0x7ff00000;
+// a Chebyshev step below 2^-18 |X| leaves an error of order |dX / X|^3 < 2e-17: converged
+constexpr double kConv = 3.814697265625e-06;
+constexpr int kHiConv2 = 0x3db00000;  // high word of kConv^2 = 2^-36
 
 // Kepler drift of the B planets of this lane about a fixed centre of gravitational parameter mu for time tau
 // (R-M3, R-M4).  The same root as the oracle's plain Newton iteration, reached with fewer evaluations of
@@ -133,7 +136,8 @@ constexpr int kHiInf = 0x7ff00000;
 //   * each iteration is Newton's step d1 = F / F' with Chebyshev's third-order correction d1 (1 + F F'' / (2 F'^2)),
 //     F' = r, F'' = eta G0 + (mu - beta r0) G1 (derivatives of the G functions: G0' = -beta G1, G_n' = G_{n-1});
 //     the correction is dropped when it is not small, which leaves Newton's step;
-//   * when every planet's step is below 1e-6 |X| the iteration has converged to far below rounding (the error after
+//   * the iteration starts from the fourth-order series solution of the equation (below), not from X = tau / r0;
+//   * when every planet's step is below 2^-18 |X| the iteration has converged to far below rounding (the error after
 //     the step is of order |dX / X|^3), and the G functions at the final X follow from a second-order Taylor update
 //     with those same derivatives (neglected terms < 1e-18 relative) instead of one more Stumpff evaluation;
 //   * 1 / r0 comes from the reciprocal square root of |q|^2 and 1 / r from rcp_f64;
@@ -153,8 +157,23 @@ __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[
         ir0[b] = rsqrt_f64(r02);
         r0[b] = r02 * ir0[b];
         beta[b] = fma(2.0 * mu, ir0[b], -v2);
-        X[b] = tau * ir0[b];
+        // Starting value: the universal Kepler equation is the power series
+        //   tau = r0 X + eta X^2 / 2 + (mu - beta r0) X^3 / 6 - beta eta X^4 / 24 + ...
+        // and its reversion to fourth order in u = tau / r0,
+        //   X = u (1 + u (q2 + u (q3 + u q4))),   q2 = -e1 / 2,  q3 = e1^2 / 2 - k / (6 r0),
+        //   q4 = e1 (5 k / 12 + beta r0 / 24) / r0 - 5 e1^3 / 8,   e1 = eta / r0,  k = mu - beta r0,
+        // is within 1e-6 of the root for steps of a few per cent of a period (config 4: max 7e-7), so that ONE
+        // Chebyshev step reaches rounding level; the plain guess X = u (the oracle's, R-M4) needs two.  Same root.
+        // Steps too long for the series (correction not small) start from X = u.
+        const double u = tau * ir0[b];
+        const double e1 = eta[b] * ir0[b], e2 = e1 * e1, br = beta[b] * r0[b];
+        const double k = mu - br;
+        const double q3 = fma(-1.0 / 6.0, k * ir0[b], 0.5 * e2);
+        const double q4 = fma(-0.625, e2 * e1, (e1 * ir0[b]) * fma(1.0 / 24.0, br, (5.0 / 12.0) * k));
+        const double corr = u * fma(u, fma(u, q4, q3), -0.5 * e1);
+        X[b] = abs_hi(corr) < 0x3fd00000 ? fma(u, corr, u) : u;  // |corr| < 0.25
     }
+    int ok[B];
     auto iterate = [&]() -> bool {
         double X2[B], z[B];
         Stumpff cs[B];
@@ -186,20 +205,23 @@ __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[
             const double dX = fma(d1, c, d1);
             X[b] -= dX;
             d[b] = -dX;
-            conv &= (abs_hi(dX) <= abs_hi(1e-6 * X[b])) & (abs_hi(X[b]) < kHiInf);
+            // converged when the step is small relative to X AND as an angle (beta dX^2 = the square of the step in
+            // eccentric anomaly): the error left by a Chebyshev step is of the order of the cube of that angle, which
+            // for steps of many revolutions (X large) is not small just because dX / X is
+            ok[b] = (abs_hi(dX) <= abs_hi(kConv * X[b])) & (abs_hi((beta[b] * dX) * dX) <= kHiConv2) &
+                    (abs_hi(X[b]) < kHiInf);
+            conv &= ok[b];
         }
         return conv != 0;
     };
-    // Two evaluations are always needed (the second confirms convergence, and is harmless if the first already
-    // had): straight-line code for them, a loop only for the rare third and later ones.
-    bool done = false;
-#pragma unroll
-    for (int it = 0; it < 2; ++it) done = iterate();
-    for (int it = 2; it < 50 && !done; ++it) done = iterate();
+    // With the series start one evaluation is the rule (the step it yields is below kConv |X|, which confirms
+    // convergence): straight-line code for it, a loop only for the later ones (long steps, high eccentricity).
+    bool done = iterate();
+    for (int it = 1; it < 50 && !done; ++it) done = iterate();
     if (!done) {  // some planet of this lane did not converge within the cap (or went non-finite): bisect those
 #pragma unroll
         for (int b = 0; b < B; ++b) {
-            if (!((abs_hi(d[b]) <= abs_hi(1e-6 * X[b])) & (abs_hi(X[b]) < kHiInf))) {
+            if (!ok[b]) {
                 X[b] = kepler_bisect(r0[b], eta[b], mu, beta[b], tau);
                 g[b] = kepler_G(beta[b], X[b]);
                 d[b] = 0.0;
