@@ -163,9 +163,10 @@ ENS_API const char *ens_strerror(int code);
 
 /* Sizes the library chose for this handle: out[0] = padded system count of the SoA rows, out[1] = lanes
  * per system L, out[2] = bodies per lane B, out[3] = threads per block, out[4] = blocks of the last or next
- * Hermite launch, out[5] = registers per thread of that kernel, out[6] = resident blocks per SM (occupancy
- * API), out[7] = number of kernels this handle has launched so far. */
-ENS_API int ens_get_info(const ens_t *e, int64_t out[8]);
+ * step-loop launch, out[5] = registers per thread of that kernel, out[6] = resident blocks per SM (occupancy
+ * API), out[7] = number of kernels this handle has launched so far, out[8] = local-memory (stack / spill) bytes per
+ * thread of that kernel, out[9] = 1 if the last fixed-step Hermite launch ran on the time-sliced persistent grid. */
+ENS_API int ens_get_info(const ens_t *e, int64_t out[10]);
 
 /* Time (ms, CUDA events on `stream`) the last ens_integrate kernel took; waits for it to finish.
  * ESTATE if nothing was launched. */

@@ -722,7 +722,7 @@ int ens_log_read(const ens_t* e, int64_t* n_records, int64_t* n_dropped, int64_t
     return ENS_OK;
 }
 
-int ens_get_info(const ens_t* e, int64_t out[8]) {
+int ens_get_info(const ens_t* e, int64_t out[10]) {
     if (!e || !out) return ENS_EINVAL;
     ENS_ON_DEVICE(e);
     const ensd::KernelInfo* all[] = {&e->mvs, &e->hermite_adaptive, &e->hermite_carry, &e->hermite_sliced, &e->rkck,
@@ -738,11 +738,13 @@ int ens_get_info(const ens_t* e, int64_t out[8]) {
     const int64_t sys_per_warp = 32 / (ki->shape.L > 0 ? ki->shape.L : 1);
     const int64_t warps = (e->v.n_sys + sys_per_warp - 1) / sys_per_warp;
     out[4] = e->last_blocks ? e->last_blocks : (warps + threads / 32 - 1) / (threads / 32);
-    out[5] = out[6] = 0;
+    out[5] = out[6] = out[8] = 0;
+    out[9] = ki->fn == e->hermite_sliced.fn && ki->fn ? 1 : 0;
     if (ki->fn) {
         cudaFuncAttributes fa;
         CU(cudaFuncGetAttributes(&fa, ki->fn));
         out[5] = fa.numRegs;
+        out[8] = (int64_t)fa.localSizeBytes;
         int nb = 0;
         CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, ki->fn, threads, 0));
         out[6] = nb;

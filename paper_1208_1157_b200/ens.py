@@ -245,9 +245,10 @@ class Ensemble:
         _check(lib().ens_test_set_option(self._h, int(option), int(value)), "ens_test_set_option")
 
     def info(self) -> dict:
-        buf = (ctypes.c_int64 * 8)()
+        buf = (ctypes.c_int64 * 10)()
         _check(lib().ens_get_info(self._h, buf), "ens_get_info")
-        keys = ("n_pad", "lanes_per_system", "bodies_per_lane", "threads", "blocks", "regs", "blocks_per_sm", "launches")
+        keys = ("n_pad", "lanes_per_system", "bodies_per_lane", "threads", "blocks", "regs", "blocks_per_sm", "launches",
+                "stack_bytes", "sliced")
         return dict(zip(keys, list(buf)))
 
     def last_kernel_ms(self) -> float:

@@ -19,6 +19,26 @@ def test_algorithmic_work_counts_match_the_design_formulas():
         assert bench.hermite_work(n) == (3 * P * 38 + 3 * n * 17 + 3 * n + 1, 3 * P * 60 + 3 * n * 34 + 5 * n + 1)
 
 
+def test_work_models_of_the_other_kernels():
+    # the counts quoted there for the tuned shapes
+    assert bench.hermite_carry_work(3)[0] == 409 and bench.rkck_work(3)[0] == 613
+    assert bench.hermite_adaptive_work(3)[0] == 505 + 62
+    assert bench.mvs_work(4)[0] == 3 * 133 + 16 + 3 * 21 == 478 and bench.mvs_work(4, merged=True)[0] == 466
+    assert bench.rkck_adaptive_work(3)[0] > bench.rkck_work(3)[0]
+    for kind, fn in bench.WORK.items():
+        for n in range(2, 17):
+            i, f = fn(n)
+            assert 0 < i < f < 2 * i, (kind, n)  # every instruction is 1 or 2 flops
+
+
+def test_traffic_is_read_from_a_committed_profile_or_absent(tmp_path):
+    p = tmp_path / "x.txt"
+    p.write_text("# header\ndram__bytes_read.sum   24.5 Mbyte\ndram__bytes_write.sum    1.5 Mbyte\n")
+    assert abs(bench.profile_traffic(str(p)) - 26.0e6) < 1
+    p.write_text("dram__bytes_read.sum 24.5 Mbyte\n")
+    assert bench.profile_traffic(str(p)) is None and bench.profile_traffic(str(tmp_path / "missing")) is None
+
+
 def test_derived_fp64_peak():
     lane, tf = bench.nominal_fp64_peak(148, 1965.0)
     assert abs(lane - 148 * 64 * 1.965e9) < 1 and abs(tf - 37.22496) < 1e-9
@@ -43,6 +63,8 @@ def test_reference_arm_prints_one_json_line():
     assert line["impl"] == "reference" and line["metric"] == bench.METRIC and line["unit"] == "system-steps/s"
     assert line["value"] > 1e5 and line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
     assert line["config"]["workload"] == "hermite_131072x3" and line["higher_is_better"] is True
+    # one sample definition for the reference arm and the cpu_baseline leg
+    assert line["config"]["sample"] == line["cpu_baseline"]["sample"] and "x 10000 steps" in line["config"]["sample"]
     # under torchrun the other ranks exit 0 without work and without output
     out = subprocess.check_output([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
                                    "--warmup", "0"], text=True, env=dict(os.environ, RANK="1", WORLD_SIZE="2"))
