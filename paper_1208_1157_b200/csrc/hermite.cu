@@ -37,10 +37,15 @@ ENS_SHAPE(5, 1, 5, true, 64, 1, 128)
 // 0.54 for the best 3-lane shape; 32-thread blocks spread the 1024 warps of config 2 evenly over the SMs; straight-line
 // step 0.668 against 0.653 for the 3-phase loop
 ENS_SHAPE(6, 1, 6, true, 32, 1, 32)
-ENS_SHAPE(7, 3, 3, false, 64, 1, 128)
-ENS_SHAPE(8, 3, 3, false, 64, 1, 128)
+// n_body = 7, 8: still one system per thread.  The state no longer fits 255 registers (336 / 664 B of it live in
+// local memory, L1-resident: the step loop touches no other memory), yet every lane does useful work and nothing is
+// shuffled: 0.65 / 0.63 of FP64 issue peak against 0.36 / 0.46 for 3 lanes x 3 bodies (9 slots for 7 or 8 bodies).
+// From n_body = 9 on the spill traffic wins (0.44 against 0.59) and the lane-split shapes take over.
+ENS_SHAPE(7, 1, 7, false, 32, 1, 32)
+ENS_SHAPE(8, 1, 8, false, 32, 1, 32)
 ENS_SHAPE(9, 3, 3, false, 64, 1, 128)
-ENS_SHAPE(10, 5, 2, false, 64, 1, 128)
+// n_body = 10 (the paper's largest Table 3 shape): 168 registers -> 12 warps per SM: 0.60 against 0.54 at 242 registers
+ENS_SHAPE(10, 5, 2, false, 64, 3, 128)
 ENS_SHAPE(11, 3, 4, false, 64, 1, 128)
 ENS_SHAPE(12, 3, 4, false, 64, 1, 128)
 ENS_SHAPE(13, 5, 3, false, 64, 1, 128)

@@ -11,7 +11,7 @@
 //   * pairs across lanes: ring schedule.  At shift s = 1..(L-1)/2 lane l fetches the bodies of lane (l+s) mod L
 //     with warp shuffles, accumulates its own half of each pair in registers and the visitor's half (Newton's
 //     third law) in a temporary that is shuffled back to the owner.  No shared memory, no __syncthreads.
-// L = 1 (n_body <= 6) is "one system per thread" and contains no shuffle at all.
+// L = 1 (n_body <= 8) is "one system per thread" and contains no shuffle at all.
 //
 // The first evaluation of step k+1 is the evaluation of the post-step-k state, so its minimum pair distance IS
 // the close-approach monitor Alg. 1 places after step k: monitors cost no extra pair work, and a

@@ -15,7 +15,7 @@
 //
 // Work split: L lanes per system (L odd), B planets per lane; the Kepler drift is per planet and needs no
 // communication; planet-planet pairs use the same in-lane + ring-of-shuffles schedule as the Hermite kernel; the
-// momentum sum of the Cartesian drift is an L-lane all-gather of per-lane partial sums.  L = 1 (n_body <= 6) is
+// momentum sum of the Cartesian drift is an L-lane all-gather of per-lane partial sums.  L = 1 (n_body <= 9) is
 // one system per thread with the oracle's summation order and no shuffle.
 #pragma once
 #include <cfloat>
