@@ -219,8 +219,9 @@ def cpu_baseline(budget_s: float = 12.0):
         taken += run()
         passes += 1
     dt = time.perf_counter() - t0
-    return {"value": taken / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{desc}; {passes} passes, {dt:.1f} s wall"}
+    return {"value": taken / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+            "passes": passes, "wall_s": dt,
+            "note": "the correctness oracle as it stands (plain loops, -O2, no FMA contraction): a reported baseline, not a tuned CPU code"}
 
 
 def run_reference(args):

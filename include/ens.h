@@ -19,6 +19,9 @@
  *     Host-space calls enqueue the copies on `stream` and then wait for it, so the host buffers are complete (get)
  *     or reusable (set) on return; the first one also allocates the device staging area, unless
  *     ens_reserve_host_staging did so before.
+ *   - Work enqueued for ONE handle must be stream-ordered: use one stream per handle, or order the streams yourself
+ *     (the handle's state rows, work counters and staging are shared by its calls).  Different handles are independent
+ *     and may run concurrently on different streams.
  *   - Every call runs on the CUDA device that was current when the handle was created, whatever device is current
  *     in the calling thread, and leaves the caller's current device unchanged.  Pointers and streams passed to a
  *     call must belong to that device.
