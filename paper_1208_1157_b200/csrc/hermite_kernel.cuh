@@ -26,6 +26,8 @@ namespace ensd {
 // One unordered pair (i, k): adds m_k f to (a_i, j_i) and -m_i f to (a_k, j_k), with
 //   f_a = dx / r^3,  f_j = (dv - 3 (dx.dv) dx / r^2) / r^3,  dx = x_k - x_i, dv = v_k - v_i   (Eq. 1 and d/dt, R1-R2).
 // 38 FP64 instructions.  r2 is returned for the close-approach monitor.
+// FIRST_K = true: (a_k, j_k) are assigned, not accumulated (the visitor's sums start with this pair: saves clearing them).
+template <bool FIRST_K = false>
 __device__ __forceinline__ double pair_acc_jerk(const double (&xi)[3], const double (&vi)[3], double mi,
                                                 double (&ai)[3], double (&ji)[3], const double (&xk)[3],
                                                 const double (&vk)[3], double mk, double (&ak)[3],
@@ -49,8 +51,13 @@ __device__ __forceinline__ double pair_acc_jerk(const double (&xi)[3], const dou
         u[c] = fma(s3, dx[c], dv[c]);
         ai[c] = fma(wi, dx[c], ai[c]);
         ji[c] = fma(wi, u[c], ji[c]);
-        ak[c] = fma(wk, dx[c], ak[c]);
-        jk[c] = fma(wk, u[c], jk[c]);
+        if constexpr (FIRST_K) {
+            ak[c] = wk * dx[c];
+            jk[c] = wk * u[c];
+        } else {
+            ak[c] = fma(wk, dx[c], ak[c]);
+            jk[c] = fma(wk, u[c], jk[c]);
+        }
     }
     return r2;
 }
@@ -130,12 +137,14 @@ __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const dou
 #pragma unroll
             for (int c = 0; c < B; ++c) {
                 if (s < H) fetch_body(s + 1, c, buf ^ 1);
-                double av[3] = {0.0, 0.0, 0.0}, jv[3] = {0.0, 0.0, 0.0};
+                double av[3], jv[3];  // the visitor's half of these B pairs: started by the first pair
                 const bool vvalid = !PADDED || (ls * B + c < N);
 #pragma unroll
                 for (int b = 0; b < B; ++b) {
-                    const double r2 = pair_acc_jerk(x[b], v[b], m[b], a[b], j[b], xv[buf][c], vv[buf][c], mv[buf][c],
-                                                    av, jv);
+                    const double r2 = b == 0 ? pair_acc_jerk<true>(x[b], v[b], m[b], a[b], j[b], xv[buf][c], vv[buf][c],
+                                                                   mv[buf][c], av, jv)
+                                             : pair_acc_jerk(x[b], v[b], m[b], a[b], j[b], xv[buf][c], vv[buf][c],
+                                                             mv[buf][c], av, jv);
                     if constexpr (TRACK) min_hi(r2min, r2, vvalid && (!PADDED || (l * B + b < N)));
                 }
                 if (c > 0) add_returns(c - 1);  // sent one visitor body ago
