@@ -130,7 +130,10 @@ cudaError_t launch_n(const View& v, StepArgs a, const LaunchTune& tune, cudaStre
             if (tune.slice_steps <= 0 && k < 32) k = 32;
             if (k > a.max_steps) k = a.max_steps;
             a.slice_steps = k;
+            // at most 256 slices: the last one is open-ended (it runs whatever is left of max_steps), so a huge step
+            // budget with a time limit (max_steps = 10^9, t_end = 20) does not turn into millions of empty tasks
             a.n_slices = (a.max_steps + k - 1) / k;
+            if (a.n_slices > 256) a.n_slices = 256;
             a.n_groups = warps;
             if (blocks > resident) blocks = resident;
             if ((err = cudaMemsetAsync(a.counter, 0, sizeof(unsigned long long), s)) != cudaSuccess) return err;

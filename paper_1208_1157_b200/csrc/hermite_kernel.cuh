@@ -563,7 +563,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 if (s > 0 && st == ENS_DONE_TIME) active = writeback = false;
             }
             const int64_t left = p.max_steps - s * p.slice_steps;
-            kmax = left < p.slice_steps ? left : p.slice_steps;
+            kmax = (left < p.slice_steps || s == p.n_slices - 1) ? left : p.slice_steps;  // the last slice is open-ended
             run();
             store_system();
             __threadfence();

@@ -67,6 +67,28 @@ def test_sliced_monitors_time_limit_and_sticky_stops():
     assert (ref["status"] == o["status"]).all() and (ref["nsteps"] == o["nsteps"]).all() and (ref["time"] == o["time"]).all()
 
 
+def test_huge_step_budget_with_a_time_limit_stays_cheap_when_sliced():
+    """max_steps = 10^9 with t_end deciding the run: the slice count is capped (the last slice is open-ended), so the
+    launch does not hand out millions of empty tasks; results equal the one-pass kernel's, also when the steps needed
+    exceed 256 slices' worth (systems that start far before t_end)."""
+    import time as _time
+    n_sys = 1531
+    pos, vel, mass = _random_systems(n_sys, 15, 77)
+    t0 = np.where(np.arange(n_sys) % 5 == 0, -3.0, 0.0)  # every fifth system needs 4x the steps of the others
+    with ens.Ensemble(n_sys, 15) as e:
+        e.set_option(ens.OPT_SLICE_MODE, 2)
+        ref = _run(e, pos, vel, mass, 0.004, 10**9, t_end=1.0, time=t0)
+        for slice_steps in (0, 1, 3):  # 0: the library's choice; 1, 3: 256 slices cover only 256 / 768 of the 250 / 1000 steps
+            e.set_option(ens.OPT_SLICE_MODE, 1)
+            e.set_option(ens.OPT_SLICE_STEPS, slice_steps)
+            w0 = _time.perf_counter()
+            got = _run(e, pos, vel, mass, 0.004, 10**9, t_end=1.0, time=t0)
+            assert _time.perf_counter() - w0 < 20.0
+            for k in KEYS:
+                assert (got[k] == ref[k]).all(), (k, slice_steps)
+    assert (ref["status"] == ens.DONE_TIME).all() and set(ref["nsteps"]) == {250, 1000}
+
+
 def test_library_chooses_slicing_for_config3_and_results_match_the_oracle():
     """Config 3 at full size (1.15 waves of resident warps) is the case the sliced grid exists for: the library's own
     choice must pick it, and sampled systems agree with the oracle (short run: the full run is test_gpu_hermite's)."""
