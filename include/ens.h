@@ -143,7 +143,9 @@ ENS_API int ens_log_enable(ens_t *e, int64_t capacity, void *stream);
  * no host round trip between segments.  Records beyond the capacity are dropped and counted.  Results are
  * bit-identical to one ens_integrate of max_steps for ENS_HERMITE, ENS_HERMITE_ADAPTIVE, ENS_RKCK and ENS_MVS up to
  * its coordinate round trip (their step is a pure function of the state); ENS_HERMITE_CARRY re-evaluates at every
- * segment start.  EINVAL: as ens_integrate, or log_every < 1, or no ENS_LOG_* bit.  ESTATE: no log buffer / state. */
+ * segment start.  EINVAL: as ens_integrate, or log_every < 1, or no ENS_LOG_* bit, or more than 10^6 segments
+ * (max_steps / log_every: every segment is enqueued from the host whether or not systems still run).
+ * ESTATE: no log buffer / state. */
 ENS_API int ens_integrate_logged(ens_t *e, int integrator, double dt, double t_end, int64_t max_steps,
                                  int64_t log_every, int what, void *stream);
 

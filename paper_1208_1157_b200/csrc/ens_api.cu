@@ -678,6 +678,9 @@ int ens_log_enable(ens_t* e, int64_t capacity, void* stream) {
 int ens_integrate_logged(ens_t* e, int integrator, double dt, double t_end, int64_t max_steps, int64_t log_every,
                          int what, void* stream) {
     if (!e || log_every < 1 || !(what & (ENS_LOG_SNAPSHOTS | ENS_LOG_STOPS))) return ENS_EINVAL;
+    // every segment is two launches enqueued from the host, whether or not systems are still running: a step budget
+    // that is really "until t_end" must come with a log_every that keeps the segment count sane
+    if (max_steps / log_every > 1000000) return ENS_EINVAL;
     if (e->log.capacity == 0) return ENS_ESTATE;
     ENS_ON_DEVICE(e);
     cudaStream_t s = (cudaStream_t)stream;

@@ -81,3 +81,8 @@ def test_log_argument_checks():
                 e.integrate_logged(ens.HERMITE, 0.01, 10, **{"log_every": 5, **bad})
         with pytest.raises(ens.EnsError):
             e.log_enable(-1)
+        with pytest.raises(ens.EnsError):  # 10^9 steps in segments of 100: ten million segments would be enqueued
+            e.integrate_logged(ens.HERMITE, 0.01, 10**9, 100, t_end=1.0)
+        e.integrate_logged(ens.HERMITE, 0.01, 10**5, 10**4, t_end=1.0)  # 10 segments; t_end ends the run in the first
+        st = e.get_state()
+        assert (st["status"] == ens.DONE_TIME).all() and (st["nsteps"] == 100).all()
