@@ -299,7 +299,11 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
     int64_t sys = warp * S + sl;
 
     double X[B][3], V[B][3], m[B];
-    double t = 0.0;
+    // Time is kept folded with the direction of the run: ts = t going forward, -t going backward (negation is exact,
+    // so ts += |h| mirrors t += h bit for bit) and the end test is the one comparison ts < te in both directions.
+    const bool fwd = p.dt > 0.0;
+    const double te = fwd ? p.t_end : -p.t_end;
+    double ts = 0.0;
     int st = ENS_STOP_NONFINITE;
     bool active = false, writeback = false;
     int64_t k = 0;
@@ -328,7 +332,10 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 m[b] = e.mass[(int64_t)gid * e.n_pad + sys];
             }
         }
-        t = ld(&e.time[sys]);
+        {
+            const double t = ld(&e.time[sys]);
+            ts = fwd ? t : -t;
+        }
         st = ld(&e.status[sys]);
         k = 0;
         active = st < ENS_STOP_CLOSE;  // STOP_* are sticky; DONE_* run again
@@ -348,7 +355,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 }
             }
             if (l == 0) {
-                e.time[sys] = t;
+                e.time[sys] = fwd ? ts : -ts;
                 e.status[sys] = st;
                 e.nsteps[sys] = ld(&e.nsteps[sys]) + k;
             }
@@ -393,7 +400,6 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
     //   x_c = C_x + 3/20 h^2 a1 - 1/30 h^3 j1        v_c = C_v + h/2 a1 - 1/12 h^2 j1
     // The ten coefficients come precomputed in StepArgs (constant bank operands of the DFMAs: no registers).
     double h = p.dt;  // the step taken; ADAPT: recomputed from (a0, j0) at the start of every step
-    const bool fwd = p.dt > 0.0;
 
     double Cx[B][3], Cv[B][3];
     double a[B][3], j[B][3];
@@ -401,21 +407,37 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
 
     // phase 0 of the loop below; returns with `active` updated.  X, V hold the accepted state.
     auto accept_and_predict = [&](unsigned amask) {
-        {  // monitors act on post-step states only (Alg. 1: advance, then execute(M)).  Every active lane takes part
-           // in the flag reduction (with refilled systems k differs between the systems of a warp).
+        // Monitors act on post-step states only (Alg. 1: advance, then execute(M)).  Nearly every step of nearly every
+        // system has nothing to report, so the step loop carries ONE test and one warp-uniform, almost never taken
+        // branch: a lane is `quiet` when every pair it saw is farther apart than r_close and every body it owns is
+        // nearer than r_eject, judged on the high words of the squared distances (strictly beyond the threshold's
+        // high word on the safe side: the exact 64-bit decision cannot differ; non-finite values sort above every
+        // finite one), and `go` when it is quiet, has time left and steps left.  Only when some lane of the warp is not
+        // `go` does the warp run the exact monitor / stop logic (which also resolves high-word ties).
+        unsigned dmax = 0u;  // largest high word of |x_b|^2 over the bodies of this lane
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            const double d2 = fma(X[b][2], X[b][2], fma(X[b][1], X[b][1], X[b][0] * X[b][0]));
+            if (!PADDED || (l * B + b < N)) dmax = max(dmax, (unsigned)__double2hiint(d2));
+        }
+        const bool go = (r2min > (unsigned)(p.rc2_bits >> 32)) && (dmax < (unsigned)(p.re2_bits >> 32)) && (ts < te) &&
+                        (k < kmax);
+        if (__ballot_sync(amask, !go) != 0u) {
+            // every active lane takes part in the flag reduction (with refilled systems k differs between the
+            // systems of a warp)
             const int f = monitor_flags<N, L, B>(X, r2min, p, l, base, amask);
             if (k > 0 && f) {
                 st = (f & 4) ? ENS_STOP_NONFINITE : (f & 1) ? ENS_STOP_CLOSE : ENS_STOP_EJECT;
                 active = false;
             }
-        }
-        if (active) {
-            if (!(fwd ? (t < p.t_end) : (t > p.t_end))) {
-                st = ENS_DONE_TIME;
-                active = false;
-            } else if (k >= kmax) {
-                st = ENS_DONE_STEPS;
-                active = false;
+            if (active) {
+                if (!(ts < te)) {
+                    st = ENS_DONE_TIME;
+                    active = false;
+                } else if (k >= kmax) {
+                    st = ENS_DONE_STEPS;
+                    active = false;
+                }
             }
         }
         // lanes that just stopped take no part in the shuffles below: re-vote (every lane of amask is here)
@@ -489,7 +511,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                     correct();
                     eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am2);
                     correct();
-                    t += h;
+                    ts += fabs(h);  // h carries the sign of the direction
                     ++k;
                 }
             }
@@ -519,7 +541,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 } else {
                     correct();
                     if (phase == 2) {
-                        t += h;
+                        ts += fabs(h);  // h carries the sign of the direction
                         ++k;
                     }
                 }
