@@ -543,12 +543,20 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
     ensd::StepArgs a{};
     a.dt = dt;
     a.t_end = t_end;
+    a.te = dt > 0.0 ? t_end : -t_end;
     a.max_steps = max_steps;
     const double rc2 = e->r_close * e->r_close;
     double re2 = e->r_eject * e->r_eject;
     if (!(re2 < DBL_MAX)) re2 = DBL_MAX;
     memcpy(&a.rc2_bits, &rc2, 8);
     memcpy(&a.re2_bits, &re2, 8);
+    {   // coordinate filter of the step loops' quick test: |x_c| < ce for all three components => |x|^2 < re2, with a
+        // margin of one high-word unit (2^-20 relative) against the rounding of the exact sum
+        const double ce = std::sqrt(re2 / 3.0);
+        unsigned long long b;
+        memcpy(&b, &ce, 8);
+        a.ce_hi = (unsigned)(b >> 32) - 1u;
+    }
     ensd::fill_step_constants(a);
     a.counter = e->counter;
     a.order = nullptr;

@@ -28,9 +28,11 @@ struct View {
 struct StepArgs {
     double dt;
     double t_end;
+    double te;  // t_end folded with the direction of the run: t_end going forward (dt > 0), -t_end going backward
     int64_t max_steps;
     unsigned long long rc2_bits;  // bit pattern of r_close^2 (0 when the monitor is off)
     unsigned long long re2_bits;  // bit pattern of min(r_eject^2, DBL_MAX): also catches inf / NaN positions
+    unsigned ce_hi;  // quick test: a body whose three |coordinates| all have a high word below this is inside r_eject
     // Step-size powers of Eq. 3 / Eq. 4 folded into per-launch constants (hermite_kernel.cuh), computed once on the
     // host in IEEE double and read by the kernels straight from the constant bank (no registers held across the loop):
     //   x_p = x + h v + p_a a0 + p_j j0              v_p = v + h a0 + p_a j0

@@ -300,9 +300,8 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
 
     double X[B][3], V[B][3], m[B];
     // Time is kept folded with the direction of the run: ts = t going forward, -t going backward (negation is exact,
-    // so ts += |h| mirrors t += h bit for bit) and the end test is the one comparison ts < te in both directions.
+    // so ts += |h| mirrors t += h bit for bit) and the end test is the one comparison ts < p.te in both directions.
     const bool fwd = p.dt > 0.0;
-    const double te = fwd ? p.t_end : -p.t_end;
     double ts = 0.0;
     int st = ENS_STOP_NONFINITE;
     bool active = false, writeback = false;
@@ -409,20 +408,20 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
     auto accept_and_predict = [&](unsigned amask) {
         // Monitors act on post-step states only (Alg. 1: advance, then execute(M)).  Nearly every step of nearly every
         // system has nothing to report, so the step loop carries ONE test and one warp-uniform, almost never taken
-        // branch: a lane is `quiet` when every pair it saw is farther apart than r_close and every body it owns is
-        // nearer than r_eject, judged on the high words of the squared distances (strictly beyond the threshold's
-        // high word on the safe side: the exact 64-bit decision cannot differ; non-finite values sort above every
-        // finite one), and `go` when it is quiet, has time left and steps left.  Only when some lane of the warp is not
+        // branch: a lane is `quiet` when every pair it saw is farther apart than r_close (high word of r^2 strictly
+        // above the threshold's: the exact 64-bit decision cannot differ) and every coordinate of its bodies is below
+        // r_eject / sqrt(3) (high words of the coordinates, integer ALU; StepArgs::ce_hi: then |x|^2 < r_eject^2 and
+        // finite; non-finite values sort above every finite one), and `go` when it is quiet, has time left and steps
+        // left.  Only when some lane of the warp is not
         // `go` does the warp run the exact monitor / stop logic (which also resolves high-word ties).
-        unsigned dmax = 0u;  // largest high word of |x_b|^2 over the bodies of this lane
+        unsigned cmax = 0u;  // largest high word of the |coordinates| of the bodies of this lane (integer ALU)
 #pragma unroll
-        for (int b = 0; b < B; ++b) {
-            const double d2 = fma(X[b][2], X[b][2], fma(X[b][1], X[b][1], X[b][0] * X[b][0]));
-            if (!PADDED || (l * B + b < N)) dmax = max(dmax, (unsigned)__double2hiint(d2));
-        }
-        const bool go = (r2min > (unsigned)(p.rc2_bits >> 32)) && (dmax < (unsigned)(p.re2_bits >> 32)) && (ts < te) &&
-                        (k < kmax);
-        if (__ballot_sync(amask, !go) != 0u) {
+        for (int b = 0; b < B; ++b)
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+                if (!PADDED || (l * B + b < N)) cmax = max(cmax, (unsigned)__double2hiint(X[b][c]) & 0x7fffffffu);
+        const bool go = (r2min > (unsigned)(p.rc2_bits >> 32)) && (cmax < p.ce_hi) && (ts < p.te) && (k < kmax);
+        if (__builtin_expect(__ballot_sync(amask, !go) != 0u, 0)) {
             // every active lane takes part in the flag reduction (with refilled systems k differs between the
             // systems of a warp)
             const int f = monitor_flags<N, L, B>(X, r2min, p, l, base, amask);
@@ -431,7 +430,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 active = false;
             }
             if (active) {
-                if (!(ts < te)) {
+                if (!(ts < p.te)) {
                     st = ENS_DONE_TIME;
                     active = false;
                 } else if (k >= kmax) {
