@@ -33,6 +33,9 @@ struct StepArgs {
     unsigned long long rc2_bits;  // bit pattern of r_close^2 (0 when the monitor is off)
     unsigned long long re2_bits;  // bit pattern of min(r_eject^2, DBL_MAX): also catches inf / NaN positions
     unsigned ce_hi;  // quick test: a body whose three |coordinates| all have a high word below this is inside r_eject
+    // MVS quick test (heliocentric Q, centre of mass Xcm): |Q_c| < ce / 4 and |Xcm_c| < ce / 2 bound every barycentric
+    // coordinate by ce; a planet with some |Q_c| > r_close is farther than r_close from the star
+    unsigned ceq_hi, cex_hi, rc1_hi;
     // Step-size powers of Eq. 3 / Eq. 4 folded into per-launch constants (hermite_kernel.cuh), computed once on the
     // host in IEEE double and read by the kernels straight from the constant bank (no registers held across the loop):
     //   x_p = x + h v + p_a a0 + p_j j0              v_p = v + h a0 + p_a j0

@@ -304,7 +304,9 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
 
     double Q[B][3], V[B][3], A[B][3], m[B];
     double Xcm[3] = {0.0, 0.0, 0.0}, Vcm[3] = {0.0, 0.0, 0.0};
-    double m0 = 1.0, im0 = 1.0, Mtot = 1.0, t = 0.0;
+    // time folded with the direction of the run (ts = t forward, -t backward: exact), end test ts < p.te either way
+    const bool fwd = p.dt > 0.0;
+    double m0 = 1.0, im0 = 1.0, Mtot = 1.0, ts = 0.0;
     int st = ENS_STOP_NONFINITE;
     bool active = false;
 #pragma unroll
@@ -318,7 +320,7 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
     if (live) {
         st = e.status[sys];
         active = st < ENS_STOP_CLOSE;  // STOP_* are sticky; DONE_* run again
-        t = e.time[sys];
+        ts = fwd ? e.time[sys] : -e.time[sys];
         // to_dh: total mass and centre of mass over all bodies in index order; every lane of the system reads all
         // bodies (L1-resident, once per launch) so that the sums need no communication
         double x0[3], sx[3] = {0.0, 0.0, 0.0}, sv[3] = {0.0, 0.0, 0.0};
@@ -359,7 +361,6 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
     const bool writeback = active;
 
     const double h = p.dt, hh = 0.5 * p.dt;
-    const bool fwd = h > 0.0;
     const bool mon_close = p.rc2_bits != 0ull;
     const bool mon_eject = p.re2_bits < 0x7FEFFFFFFFFFFFFFull;
     int64_t k = 0;
@@ -368,7 +369,7 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
 
     // Alg. 1 loop test before the first step (R10): time first, then the step budget
     if (active) {
-        if (!(fwd ? (t < p.t_end) : (t > p.t_end))) {
+        if (!(ts < p.te)) {
             st = ENS_DONE_TIME;
             active = false;
         } else if (k >= p.max_steps) {
@@ -452,59 +453,80 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
                     Xp[c] = fma(hh, Vcm[c], Xcm[c]);
                 }
             }
-            t += h;
+            ts += fabs(h);
             ++k;
             const double(&Qm)[B][3] = MERGED ? Qp : Q;  // the post-step positions
             const double(&Xm)[3] = MERGED ? Xp : Xcm;
 
-            // monitors on the post-step state (Alg. 1 execute(M); R11).  Planet-planet separations are
-            // those of the acceleration evaluation: the drift shifts every planet alike.
-            int f = 0;
-            if (mon_close && r2min < p.rc2_bits) f |= 1;
-            u64 q2max = 0ull, q2min = ~0ull;  // over this lane's planets: star-planet separation is |Q_i|
+            // Monitors on the post-step state (Alg. 1 execute(M); R11) and the loop tests.  One quick test per
+            // step on the integer ALU (high words): planet pairs farther apart than r_close (r2min of the acceleration
+            // evaluation: the drift shifts every planet alike), every planet with some |Q_c| > r_close (farther
+            // than that from the star), every |Q_c| < ce / 4 and |Xcm_c| < ce / 2 (then every barycentric coordinate is
+            // below ce = r_eject / sqrt(3), and everything is finite), time left, steps left.  The exact logic runs only
+            // when some lane of the warp fails it (warp-uniform, rarely taken).
+            unsigned qhi = 0u, qlo = ~0u;
 #pragma unroll
             for (int b = 0; b < B; ++b) {
                 if (!PADDED || (l * B + b < P)) {
-                    const u64 q2 = dbits(fma(Qm[b][2], Qm[b][2], fma(Qm[b][1], Qm[b][1], Qm[b][0] * Qm[b][0])));
-                    q2max = q2 > q2max ? q2 : q2max;
-                    q2min = q2 < q2min ? q2 : q2min;
+                    const unsigned m3 = max(max((unsigned)__double2hiint(Qm[b][0]) & 0x7fffffffu,
+                                                (unsigned)__double2hiint(Qm[b][1]) & 0x7fffffffu),
+                                            (unsigned)__double2hiint(Qm[b][2]) & 0x7fffffffu);
+                    qhi = max(qhi, m3);
+                    qlo = min(qlo, m3);
                 }
             }
-            if (q2max > 0x7FEFFFFFFFFFFFFFull) f |= 4;  // +inf or NaN
-            if (q2min < p.rc2_bits) f |= 1;
-            if (mon_eject) {  // distances from the coordinate origin need the star's barycentric position
-                double sq[3], x0[3];
-                mass_weighted_sum<L, B>(Qm, m, sq, l, base, amask);
-#pragma unroll
-                for (int c = 0; c < 3; ++c) x0[c] = Xm[c] - sq[c] / Mtot;
-                if (dbits(fma(x0[2], x0[2], fma(x0[1], x0[1], x0[0] * x0[0]))) > p.re2_bits) f |= 2;
+            const unsigned xhi = max(max((unsigned)__double2hiint(Xm[0]) & 0x7fffffffu, (unsigned)__double2hiint(Xm[1]) & 0x7fffffffu),
+                                     (unsigned)__double2hiint(Xm[2]) & 0x7fffffffu);
+            const bool go = ((unsigned)(r2min >> 32) > (unsigned)(p.rc2_bits >> 32)) && (qlo > p.rc1_hi) && (qhi < p.ceq_hi) &&
+                            (xhi < p.cex_hi) && (ts < p.te) && (k < p.max_steps);
+            if (__builtin_expect(__ballot_sync(amask, !go) != 0u, 0)) {
+                int f = 0;
+                if (mon_close && r2min < p.rc2_bits) f |= 1;
+                u64 q2max = 0ull, q2min = ~0ull;  // over this lane's planets: star-planet separation is |Q_i|
 #pragma unroll
                 for (int b = 0; b < B; ++b) {
                     if (!PADDED || (l * B + b < P)) {
-                        const double xx = x0[0] + Qm[b][0], yy = x0[1] + Qm[b][1], zz = x0[2] + Qm[b][2];
-                        if (dbits(fma(zz, zz, fma(yy, yy, xx * xx))) > p.re2_bits) f |= 2;
+                        const u64 q2 = dbits(fma(Qm[b][2], Qm[b][2], fma(Qm[b][1], Qm[b][1], Qm[b][0] * Qm[b][0])));
+                        q2max = q2 > q2max ? q2 : q2max;
+                        q2min = q2 < q2min ? q2 : q2min;
                     }
                 }
-            }
-            if constexpr (L > 1) {
-                int g = f;
+                if (q2max > 0x7FEFFFFFFFFFFFFFull) f |= 4;  // +inf or NaN
+                if (q2min < p.rc2_bits) f |= 1;
+                if (mon_eject) {  // distances from the coordinate origin need the star's barycentric position
+                    double sq[3], x0[3];
+                    mass_weighted_sum<L, B>(Qm, m, sq, l, base, amask);
 #pragma unroll
-                for (int i = 1; i < L; ++i) {
-                    int li = l + i;
-                    if (li >= L) li -= L;
-                    g |= __shfl_sync(amask, f, base + li);
+                    for (int c = 0; c < 3; ++c) x0[c] = Xm[c] - sq[c] / Mtot;
+                    if (dbits(fma(x0[2], x0[2], fma(x0[1], x0[1], x0[0] * x0[0]))) > p.re2_bits) f |= 2;
+#pragma unroll
+                    for (int b = 0; b < B; ++b) {
+                        if (!PADDED || (l * B + b < P)) {
+                            const double xx = x0[0] + Qm[b][0], yy = x0[1] + Qm[b][1], zz = x0[2] + Qm[b][2];
+                            if (dbits(fma(zz, zz, fma(yy, yy, xx * xx))) > p.re2_bits) f |= 2;
+                        }
+                    }
                 }
-                f = g;
-            }
-            if (f) {
-                st = (f & 4) ? ENS_STOP_NONFINITE : (f & 1) ? ENS_STOP_CLOSE : ENS_STOP_EJECT;
-                active = false;
-            } else if (!(fwd ? (t < p.t_end) : (t > p.t_end))) {
-                st = ENS_DONE_TIME;
-                active = false;
-            } else if (k >= p.max_steps) {
-                st = ENS_DONE_STEPS;
-                active = false;
+                if constexpr (L > 1) {
+                    int g = f;
+#pragma unroll
+                    for (int i = 1; i < L; ++i) {
+                        int li = l + i;
+                        if (li >= L) li -= L;
+                        g |= __shfl_sync(amask, f, base + li);
+                    }
+                    f = g;
+                }
+                if (f) {
+                    st = (f & 4) ? ENS_STOP_NONFINITE : (f & 1) ? ENS_STOP_CLOSE : ENS_STOP_EJECT;
+                    active = false;
+                } else if (!(ts < p.te)) {
+                    st = ENS_DONE_TIME;
+                    active = false;
+                } else if (k >= p.max_steps) {
+                    st = ENS_DONE_STEPS;
+                    active = false;
+                }
             }
             if constexpr (MERGED) {
                 if (active) {  // full kick and full drift: the closing halves of this step and the opening ones of the next
@@ -560,7 +582,7 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
                 e.pos[(int64_t)c * e.n_pad + sys] = x0[c];
                 e.vel[(int64_t)c * e.n_pad + sys] = v0[c];
             }
-            e.time[sys] = t;
+            e.time[sys] = fwd ? ts : -ts;
             e.status[sys] = st;
             e.nsteps[sys] += k;
         }

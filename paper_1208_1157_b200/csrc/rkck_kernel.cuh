@@ -40,7 +40,9 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
     const bool live = (sl < S) && (sys < e.n_sys);
 
     double X[B][3], V[B][3], m[B];
-    double t = 0.0;
+    // time folded with the direction of the run (ts = t forward, -t backward: exact), end test ts < p.te either way
+    const bool fwd = p.dt > 0.0;
+    double ts = 0.0;
     int st = ENS_STOP_NONFINITE;
     bool active = false;
 #pragma unroll
@@ -64,13 +66,12 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
                 m[b] = e.mass[(int64_t)gid * e.n_pad + sys];
             }
         }
-        t = e.time[sys];
+        ts = fwd ? e.time[sys] : -e.time[sys];
         st = e.status[sys];
         active = st < ENS_STOP_CLOSE;  // STOP_* are sticky; DONE_* run again
     }
     const bool writeback = active;
     const double h = p.dt;
-    const bool fwd = h > 0.0;
     int64_t k = 0;
     double K[5][B][3];  // stage accelerations k_1 .. k_5
     u64 r2min;
@@ -81,13 +82,24 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
         if (active) {
             // stage 1 at the accepted state: also the monitors' pair distances (Alg. 1: advance, then execute(M))
             eval_acc_planets<N, L, B>(X, m, K[0], r2min, l, base, amask);
-            {
-                constexpr bool PADDED2 = PADDED;
+            // One quick test per step (as in hermite_kernel.cuh): every pair this lane saw farther apart than r_close and
+            // every coordinate of its bodies below r_eject / sqrt(3), both on high words (the exact decisions cannot
+            // differ; non-finite values fail it), time left, steps left.  The exact monitor / stop logic runs only when
+            // some lane of the warp fails it (warp-uniform, rarely taken).
+            unsigned cmax = 0u;
+#pragma unroll
+            for (int b = 0; b < B; ++b)
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                    if (!PADDED || (l * B + b < N)) cmax = max(cmax, (unsigned)__double2hiint(X[b][c]) & 0x7fffffffu);
+            const bool go = ((unsigned)(r2min >> 32) > (unsigned)(p.rc2_bits >> 32)) && (cmax < p.ce_hi) && (ts < p.te) &&
+                            (k < p.max_steps);
+            if (__builtin_expect(__ballot_sync(amask, !go) != 0u, 0)) {
                 int f = (r2min < p.rc2_bits) ? 1 : 0;
 #pragma unroll
                 for (int b = 0; b < B; ++b) {
                     const u64 db = dbits(fma(X[b][2], X[b][2], fma(X[b][1], X[b][1], X[b][0] * X[b][0])));
-                    if (!PADDED2 || (l * B + b < N)) {
+                    if (!PADDED || (l * B + b < N)) {
                         if (db > p.re2_bits) f |= 2;
                         if (db > 0x7FEFFFFFFFFFFFFFull) f |= 4;  // +inf or NaN
                     }
@@ -106,14 +118,14 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
                     st = (f & 4) ? ENS_STOP_NONFINITE : (f & 1) ? ENS_STOP_CLOSE : ENS_STOP_EJECT;
                     active = false;
                 }
-            }
-            if (active) {
-                if (!(fwd ? (t < p.t_end) : (t > p.t_end))) {
-                    st = ENS_DONE_TIME;
-                    active = false;
-                } else if (k >= p.max_steps) {
-                    st = ENS_DONE_STEPS;
-                    active = false;
+                if (active) {
+                    if (!(ts < p.te)) {
+                        st = ENS_DONE_TIME;
+                        active = false;
+                    } else if (k >= p.max_steps) {
+                        st = ENS_DONE_STEPS;
+                        active = false;
+                    }
                 }
             }
             // lanes that just stopped take no part in the shuffles of the remaining stages
@@ -151,7 +163,7 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
                         w = fma(q.hb[3], K[3][b][c], w);
                         V[b][c] = fma(q.hb[5], K6[b][c], w);
                     }
-                t += h;
+                ts += fabs(h);
                 ++k;
             }
         }
@@ -170,7 +182,7 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
             }
         }
         if (l == 0) {
-            e.time[sys] = t;
+            e.time[sys] = fwd ? ts : -ts;
             e.status[sys] = st;
             e.nsteps[sys] += k;
         }
@@ -320,38 +332,49 @@ __global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkU
         if (active) {
             // stage 1 at the accepted state (after an accepted step or at the start of the run): also the monitors'
             // pair distances (Alg. 1: advance, then execute(M)) and the loop tests.  A rejected trial skips all this.
-            const unsigned kmask = (L > 1) ? __ballot_sync(amask, !have_k1) : amask;
+            const unsigned kmask = __ballot_sync(amask, !have_k1);  // the lanes that take stage 1 (and its quick test)
             if (!have_k1) {
                 eval_acc_planets<N, L, B>(X, m, K[0], r2min, l, base, kmask);
                 have_k1 = true;
-                int f = (r2min < p.rc2_bits) ? 1 : 0;
+                // the quick test of the fixed-step kernel; the exact logic only when some lane of kmask fails it
+                unsigned cmax = 0u;
 #pragma unroll
-                for (int b = 0; b < B; ++b) {
-                    const u64 db = dbits(fma(X[b][2], X[b][2], fma(X[b][1], X[b][1], X[b][0] * X[b][0])));
-                    if (!PADDED || (l * B + b < N)) {
-                        if (db > p.re2_bits) f |= 2;
-                        if (db > 0x7FEFFFFFFFFFFFFFull) f |= 4;
-                    }
-                }
-                if constexpr (L > 1) {
-                    int g = f;
+                for (int b = 0; b < B; ++b)
 #pragma unroll
-                    for (int i = 1; i < L; ++i) {
-                        int li = l + i;
-                        if (li >= L) li -= L;
-                        g |= __shfl_sync(kmask, f, base + li);
+                    for (int c = 0; c < 3; ++c)
+                        if (!PADDED || (l * B + b < N)) cmax = max(cmax, (unsigned)__double2hiint(X[b][c]) & 0x7fffffffu);
+                const bool go = ((unsigned)(r2min >> 32) > (unsigned)(p.rc2_bits >> 32)) && (cmax < p.ce_hi) &&
+                                (fwd ? (t < p.t_end) : (t > p.t_end)) && (k < p.max_steps);
+                if (__builtin_expect(__ballot_sync(kmask, !go) != 0u, 0)) {
+                    int f = (r2min < p.rc2_bits) ? 1 : 0;
+#pragma unroll
+                    for (int b = 0; b < B; ++b) {
+                        const u64 db = dbits(fma(X[b][2], X[b][2], fma(X[b][1], X[b][1], X[b][0] * X[b][0])));
+                        if (!PADDED || (l * B + b < N)) {
+                            if (db > p.re2_bits) f |= 2;
+                            if (db > 0x7FEFFFFFFFFFFFFFull) f |= 4;
+                        }
                     }
-                    f = g;
-                }
-                if (k > 0 && f) {
-                    st = (f & 4) ? ENS_STOP_NONFINITE : (f & 1) ? ENS_STOP_CLOSE : ENS_STOP_EJECT;
-                    active = false;
-                } else if (!(fwd ? (t < p.t_end) : (t > p.t_end))) {
-                    st = ENS_DONE_TIME;
-                    active = false;
-                } else if (k >= p.max_steps) {
-                    st = ENS_DONE_STEPS;
-                    active = false;
+                    if constexpr (L > 1) {
+                        int g = f;
+#pragma unroll
+                        for (int i = 1; i < L; ++i) {
+                            int li = l + i;
+                            if (li >= L) li -= L;
+                            g |= __shfl_sync(kmask, f, base + li);
+                        }
+                        f = g;
+                    }
+                    if (k > 0 && f) {
+                        st = (f & 4) ? ENS_STOP_NONFINITE : (f & 1) ? ENS_STOP_CLOSE : ENS_STOP_EJECT;
+                        active = false;
+                    } else if (!(fwd ? (t < p.t_end) : (t > p.t_end))) {
+                        st = ENS_DONE_TIME;
+                        active = false;
+                    } else if (k >= p.max_steps) {
+                        st = ENS_DONE_STEPS;
+                        active = false;
+                    }
                 }
             }
             unsigned am2 = amask;
