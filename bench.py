@@ -46,7 +46,7 @@ CFG = 1
 # ---------------------------------------------------------------------------------------------------------------
 PAIR_INSTR, PAIR_FLOPS = 38, 60           # one pair acc+jerk evaluation
 COMP_INSTR, COMP_FLOPS = 17, 34           # Hermite predictor + 2 correctors, per body component
-BODY_MON_INSTR, BODY_MON_FLOPS = 3, 5     # |x_i|^2 for the ejection monitor
+BODY_MON_INSTR, BODY_MON_FLOPS = 0, 0     # monitors: the step loops test high words on the integer ALU (no FP64 work)
 ACC_PAIR_INSTR, ACC_PAIR_FLOPS = 21, 32   # one pair, acceleration only (Cash-Karp stages, MVS planet pairs)
 R2_PAIR_INSTR, R2_PAIR_FLOPS = 6, 8       # one pair separation, positions only (monitor of the 2-evaluation Hermite)
 
@@ -56,7 +56,7 @@ def _pairs(n):
 
 
 def hermite_work(n_body: int):
-    """3 evaluations per step (R6): 3 P 38 + 3 N 17 + 3 N + 1."""
+    """3 evaluations per step (R6): 3 P 38 + 3 N 17 + 1 (the time update); the monitors cost no FP64 instruction."""
     p = _pairs(n_body)
     return (3 * p * PAIR_INSTR + 3 * n_body * COMP_INSTR + n_body * BODY_MON_INSTR + 1,
             3 * p * PAIR_FLOPS + 3 * n_body * COMP_FLOPS + n_body * BODY_MON_FLOPS + 1)
@@ -92,11 +92,11 @@ def rkck_adaptive_work(n_body: int):
 
 def mvs_work(n_body: int, merged: bool = False):
     """Per planet: universal-variable Kepler drift 115 (setup 16, series start 19, one Stumpff evaluation + Chebyshev
-    step 43, Taylor finish + f, g functions 37), drifts / kicks / momentum sum / |Q|^2 18 (merged: 15); per system 16
-    (merged: 13); planet pairs 21 each."""
+    step 43, Taylor finish + f, g functions 37), drifts / kicks / momentum sum 15 (merged: 12); per system 16
+    (merged: 13); planet pairs 21 each.  The monitors cost no FP64 instruction (high words, integer ALU)."""
     pl = n_body - 1
     pp = _pairs(pl)
-    per_planet_i, per_planet_f = (115 + 15, 177 + 25) if merged else (115 + 18, 177 + 29)
+    per_planet_i, per_planet_f = (115 + 12, 177 + 20) if merged else (115 + 15, 177 + 24)
     per_sys_i, per_sys_f = (13, 19) if merged else (16, 22)
     return pl * per_planet_i + per_sys_i + pp * ACC_PAIR_INSTR, pl * per_planet_f + per_sys_f + pp * ACC_PAIR_FLOPS
 

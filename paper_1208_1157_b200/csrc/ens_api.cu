@@ -555,7 +555,8 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
         const double ce = std::sqrt(re2 / 3.0);
         unsigned long long b;
         memcpy(&b, &ce, 8);
-        a.ce_hi = (unsigned)(b >> 32) - 1u;
+        a.ce_hi = (unsigned)(b >> 32);
+        a.ce_hi = a.ce_hi > 0u ? a.ce_hi - 1u : 0u;  // 0: the quick test always fails (the exact logic decides)
         a.cex_hi = a.ce_hi > 0x00400000u ? a.ce_hi - 0x00100000u : 0u;  // ce / 2, ce / 4 (0: the quick test always fails)
         a.ceq_hi = a.ce_hi > 0x00400000u ? a.ce_hi - 0x00200000u : 0u;
         memcpy(&b, &e->r_close, 8);
