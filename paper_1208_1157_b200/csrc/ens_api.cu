@@ -543,6 +543,7 @@ int ens_integrate(ens_t* e, int integrator, double dt, double t_end, int64_t max
     ensd::StepArgs a{};
     a.dt = dt;
     a.t_end = t_end;
+    a.hh = 0.5 * dt;
     a.te = dt > 0.0 ? t_end : -t_end;
     a.max_steps = max_steps;
     const double rc2 = e->r_close * e->r_close;

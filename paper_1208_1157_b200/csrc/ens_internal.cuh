@@ -28,6 +28,7 @@ struct View {
 struct StepArgs {
     double dt;
     double t_end;
+    double hh;  // dt / 2 (MVS half steps)
     double te;  // t_end folded with the direction of the run: t_end going forward (dt > 0), -t_end going backward
     int64_t max_steps;
     unsigned long long rc2_bits;  // bit pattern of r_close^2 (0 when the monitor is off)

@@ -19,6 +19,7 @@
 // one system per thread with the oracle's summation order and no shuffle.
 #pragma once
 #include <cfloat>
+#include <type_traits>
 
 #include "acc_pairs.cuh"
 
@@ -35,7 +36,9 @@ __constant__ double kStumpff[16] = {
 
 __device__ __forceinline__ void stumpff_series(double z, double& c0, double& c1, double& c2, double& c3) {
     // Horner in z; the coefficients are constant-bank operands of the DFMAs (no registers, no immediates to build)
-    double s2 = kStumpff[0], s3 = kStumpff[1];
+    // the z^7 coefficients (-1/16!, -1/17!) truncated to their high words: built with one move each instead of a
+    // constant load the first DFMA would have to wait for; their term is < 5e-21, its truncation error < 3e-27
+    double s2 = -0x1.ae7f3p-45, s3 = -0x1.952c7p-49;
 #pragma unroll
     for (int k = 1; k < 8; ++k) {
         s2 = fma(s2, z, kStumpff[2 * k]);
@@ -146,7 +149,7 @@ constexpr int kHiConv2 = 0x3db00000;  // high word of kConv^2 = 2^-36
 // valid(b) = false leaves slot b untouched (massless dummy slots of padded shapes).
 template <int B, class Valid>
 __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[B][3], double mu, double tau,
-                                                 Valid valid) {
+                                                 unsigned amask, Valid valid) {
     double r0[B], ir0[B], eta[B], beta[B], X[B], d[B];
     KeplerG g[B];
 #pragma unroll
@@ -174,7 +177,9 @@ __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[
         X[b] = abs_hi(corr) < 0x3fd00000 ? fma(u, corr, u) : u;  // |corr| < 0.25
     }
     int ok[B];
-    auto iterate = [&]() -> bool {
+    // uniform = true_type: called with all lanes of amask converged; the choice of the Stumpff path is then one vote and a
+    // warp-uniform branch (the general path returns the series' values for small arguments, bit for bit)
+    auto iterate = [&](auto uniform) -> bool {
         double X2[B], z[B];
         Stumpff cs[B];
         int zmax = 0;
@@ -184,7 +189,9 @@ __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[
             z[b] = beta[b] * X2[b];
             zmax = max(zmax, abs_hi(z[b]));
         }
-        if (zmax < kHi0p1) {
+        bool series = zmax < kHi0p1;
+        if constexpr (decltype(uniform)::value) series = __ballot_sync(amask, !series) == 0u;
+        if (__builtin_expect(series, 1)) {
 #pragma unroll
             for (int b = 0; b < B; ++b) stumpff_series(z[b], cs[b].c0, cs[b].c1, cs[b].c2, cs[b].c3);
         } else {
@@ -216,15 +223,17 @@ __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[
     };
     // With the series start one evaluation is the rule (the step it yields is below kConv |X|, which confirms
     // convergence): straight-line code for it, a loop only for the later ones (long steps, high eccentricity).
-    bool done = iterate();
-    for (int it = 1; it < 50 && !done; ++it) done = iterate();
-    if (!done) {  // some planet of this lane did not converge within the cap (or went non-finite): bisect those
+    bool done = iterate(std::true_type{});
+    if (__builtin_expect(__ballot_sync(amask, !done) != 0u, 0)) {  // warp-uniform: some lane needs more
+        for (int it = 1; it < 50 && !done; ++it) done = iterate(std::false_type{});
+        if (!done) {  // some planet of this lane did not converge within the cap (or went non-finite): bisect those
 #pragma unroll
-        for (int b = 0; b < B; ++b) {
-            if (!ok[b]) {
-                X[b] = kepler_bisect(r0[b], eta[b], mu, beta[b], tau);
-                g[b] = kepler_G(beta[b], X[b]);
-                d[b] = 0.0;
+            for (int b = 0; b < B; ++b) {
+                if (!ok[b]) {
+                    X[b] = kepler_bisect(r0[b], eta[b], mu, beta[b], tau);
+                    g[b] = kepler_G(beta[b], X[b]);
+                    d[b] = 0.0;
+                }
             }
         }
     }
@@ -360,7 +369,7 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
     }
     const bool writeback = active;
 
-    const double h = p.dt, hh = 0.5 * p.dt;
+    const double h = p.dt, hh = p.hh;
     const bool mon_close = p.rc2_bits != 0ull;
     const bool mon_eject = p.re2_bits < 0x7FEFFFFFFFFFFFFFull;
     int64_t k = 0;
@@ -401,10 +410,16 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
             }
         }
     }
-    while (true) {
-        const unsigned amask = __ballot_sync(0xffffffffu, active);
-        if (amask == 0) break;
-        if (active) {
+    // The step loop.  All systems of the warp that run enter it together (mask `am`); a system leaves it through the
+    // exact stop logic, which runs only when the quick test at the end of a step fails for some lane of the warp: the
+    // loop itself carries one vote and one warp-uniform, almost never taken branch per step.
+    const unsigned amask0 = __ballot_sync(0xffffffffu, active);
+    if (active) {
+        unsigned am = amask0;
+        while (true) {
+            // bookkeeping first: nothing below needs it before the tests at the end of the step
+            ts += fabs(h);
+            ++k;
             double Qp[B][3], Xp[3];  // MERGED: post-step positions (after the closing half drift), temporaries
             if constexpr (!MERGED) {
                 // 1 + 2: Cartesian half drift, half kick
@@ -420,22 +435,22 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
                 }
             }
             // 3: Kepler drift of every planet about mu = G m_0 (G = 1)
-            kepler_drift_all<B>(Q, V, m0, h, [&](int b) { return !PADDED || (l * B + b < P); });
+            kepler_drift_all<B>(Q, V, m0, h, am, [&](int b) { return !PADDED || (l * B + b < P); });
             if constexpr (MERGED) {
                 // drift velocity of the rest of this step and the start of the next: kicks do not change it
-                mass_weighted_sum<L, B>(V, m, s, l, base, amask);
+                mass_weighted_sum<L, B>(V, m, s, l, base, am);
 #pragma unroll
                 for (int c = 0; c < 3; ++c) s[c] = s[c] * im0;
             }
             // 4: planet-planet accelerations at the new positions, half kick
-            eval_acc_planets<P, L, B>(Q, m, A, r2min, l, base, amask);
+            eval_acc_planets<P, L, B>(Q, m, A, r2min, l, base, am);
             if constexpr (!MERGED) {
 #pragma unroll
                 for (int b = 0; b < B; ++b)
 #pragma unroll
                     for (int c = 0; c < 3; ++c) V[b][c] = fma(hh, A[b][c], V[b][c]);
                 // 5: Cartesian half drift with the new momenta
-                mass_weighted_sum<L, B>(V, m, s, l, base, amask);
+                mass_weighted_sum<L, B>(V, m, s, l, base, am);
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     s[c] = s[c] * im0;
@@ -453,8 +468,6 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
                     Xp[c] = fma(hh, Vcm[c], Xcm[c]);
                 }
             }
-            ts += fabs(h);
-            ++k;
             const double(&Qm)[B][3] = MERGED ? Qp : Q;  // the post-step positions
             const double(&Xm)[3] = MERGED ? Xp : Xcm;
 
@@ -479,7 +492,7 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
                                      (unsigned)__double2hiint(Xm[2]) & 0x7fffffffu);
             const bool go = ((unsigned)(r2min >> 32) > (unsigned)(p.rc2_bits >> 32)) && (qlo > p.rc1_hi) && (qhi < p.ceq_hi) &&
                             (xhi < p.cex_hi) && (ts < p.te) && (k < p.max_steps);
-            if (__builtin_expect(__ballot_sync(amask, !go) != 0u, 0)) {
+            if (__builtin_expect(__ballot_sync(am, !go) != 0u, 0)) {
                 int f = 0;
                 if (mon_close && r2min < p.rc2_bits) f |= 1;
                 u64 q2max = 0ull, q2min = ~0ull;  // over this lane's planets: star-planet separation is |Q_i|
@@ -495,7 +508,7 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
                 if (q2min < p.rc2_bits) f |= 1;
                 if (mon_eject) {  // distances from the coordinate origin need the star's barycentric position
                     double sq[3], x0[3];
-                    mass_weighted_sum<L, B>(Qm, m, sq, l, base, amask);
+                    mass_weighted_sum<L, B>(Qm, m, sq, l, base, am);
 #pragma unroll
                     for (int c = 0; c < 3; ++c) x0[c] = Xm[c] - sq[c] / Mtot;
                     if (dbits(fma(x0[2], x0[2], fma(x0[1], x0[1], x0[0] * x0[0]))) > p.re2_bits) f |= 2;
@@ -513,7 +526,7 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
                     for (int i = 1; i < L; ++i) {
                         int li = l + i;
                         if (li >= L) li -= L;
-                        g |= __shfl_sync(amask, f, base + li);
+                        g |= __shfl_sync(am, f, base + li);
                     }
                     f = g;
                 }
@@ -527,28 +540,31 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
                     st = ENS_DONE_STEPS;
                     active = false;
                 }
+                am = __ballot_sync(am, active);  // the systems that go on
+                if (!active) {
+                    if constexpr (MERGED) {  // the system leaves the loop: close the step
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                            for (int b = 0; b < B; ++b) {
+                                V[b][c] = fma(hh, A[b][c], V[b][c]);
+                                Q[b][c] = Qp[b][c];
+                            }
+                            Xcm[c] = Xp[c];
+                        }
+                    }
+                    break;
+                }
             }
-            if constexpr (MERGED) {
-                if (active) {  // full kick and full drift: the closing halves of this step and the opening ones of the next
+            if constexpr (MERGED) {  // full kick and full drift: the closing halves of this step and the opening ones of the next
 #pragma unroll
-                    for (int c = 0; c < 3; ++c) {
+                for (int c = 0; c < 3; ++c) {
 #pragma unroll
-                        for (int b = 0; b < B; ++b) {
-                            V[b][c] = fma(h, A[b][c], V[b][c]);
-                            Q[b][c] = fma(h, s[c], Q[b][c]);
-                        }
-                        Xcm[c] = fma(h, Vcm[c], Xcm[c]);
+                    for (int b = 0; b < B; ++b) {
+                        V[b][c] = fma(h, A[b][c], V[b][c]);
+                        Q[b][c] = fma(h, s[c], Q[b][c]);
                     }
-                } else {  // the system leaves the loop: close the step
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-#pragma unroll
-                        for (int b = 0; b < B; ++b) {
-                            V[b][c] = fma(hh, A[b][c], V[b][c]);
-                            Q[b][c] = Qp[b][c];
-                        }
-                        Xcm[c] = Xp[c];
-                    }
+                    Xcm[c] = fma(h, Vcm[c], Xcm[c]);
                 }
             }
         }
