@@ -404,67 +404,77 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
     double a[B][3], j[B][3];
     unsigned r2min;  // high word of the smallest squared pair separation seen by the last tracking evaluation
 
-    // phase 0 of the loop below; returns with `active` updated.  X, V hold the accepted state.
-    auto accept_and_predict = [&](unsigned amask) {
-        // Monitors act on post-step states only (Alg. 1: advance, then execute(M)).  Nearly every step of nearly every
-        // system has nothing to report, so the step loop carries ONE test and one warp-uniform, almost never taken
-        // branch: a lane is `quiet` when every pair it saw is farther apart than r_close (high word of r^2 strictly
-        // above the threshold's: the exact 64-bit decision cannot differ) and every coordinate of its bodies is below
-        // r_eject / sqrt(3) (high words of the coordinates, integer ALU; StepArgs::ce_hi: then |x|^2 < r_eject^2 and
-        // finite; non-finite values sort above every finite one), and `go` when it is quiet, has time left and steps
-        // left.  Only when some lane of the warp is not
-        // `go` does the warp run the exact monitor / stop logic (which also resolves high-word ties).
-        unsigned cmax = 0u;  // largest high word of the |coordinates| of the bodies of this lane (integer ALU)
+    // Phase 0 of a step, in three parts.  X, V hold the accepted state.
+    // quick_test: monitors act on post-step states only (Alg. 1: advance, then execute(M)).  Nearly every step of nearly
+    // every system has nothing to report, so the step loop carries ONE test, one vote and one warp-uniform, almost never
+    // taken branch: a lane is `quiet` when every pair it saw is farther apart than r_close (high word of r^2 strictly
+    // above the threshold's: the exact 64-bit decision cannot differ) and every coordinate of its bodies is below
+    // r_eject / sqrt(3) (high words of the coordinates, integer ALU; StepArgs::ce_hi: then |x|^2 < r_eject^2 and finite;
+    // non-finite values sort above every finite one), and `go` when it is quiet, has time left and steps left.  Returns
+    // the lanes of amask that are not `go`; only when there is one does the warp run exact_stop.
+    auto quick_test = [&](unsigned amask) -> unsigned {
+        unsigned cmax = 0u;  // largest high word of the |coordinates| of the bodies of this lane
 #pragma unroll
         for (int b = 0; b < B; ++b)
 #pragma unroll
             for (int c = 0; c < 3; ++c)
                 if (!PADDED || (l * B + b < N)) cmax = max(cmax, (unsigned)__double2hiint(X[b][c]) & 0x7fffffffu);
         const bool go = (r2min > (unsigned)(p.rc2_bits >> 32)) && (cmax < p.ce_hi) && (ts < p.te) && (k < kmax);
-        if (__builtin_expect(__ballot_sync(amask, !go) != 0u, 0)) {
-            // every active lane takes part in the flag reduction (with refilled systems k differs between the
-            // systems of a warp)
-            const int f = monitor_flags<N, L, B>(X, r2min, p, l, base, amask);
-            if (k > 0 && f) {
-                st = (f & 4) ? ENS_STOP_NONFINITE : (f & 1) ? ENS_STOP_CLOSE : ENS_STOP_EJECT;
+        return __ballot_sync(amask, !go);
+    };
+    // exact_stop: the exact monitor / stop logic (also resolves high-word ties); updates `active` and `st`.  Every lane
+    // of amask takes part in the flag reduction (with refilled systems k differs between the systems of a warp).
+    auto exact_stop = [&](unsigned amask) {
+        const int f = monitor_flags<N, L, B>(X, r2min, p, l, base, amask);
+        if (k > 0 && f) {
+            st = (f & 4) ? ENS_STOP_NONFINITE : (f & 1) ? ENS_STOP_CLOSE : ENS_STOP_EJECT;
+            active = false;
+        }
+        if (active) {
+            if (!(ts < p.te)) {
+                st = ENS_DONE_TIME;
+                active = false;
+            } else if (k >= kmax) {
+                st = ENS_DONE_STEPS;
                 active = false;
             }
-            if (active) {
-                if (!(ts < p.te)) {
-                    st = ENS_DONE_TIME;
-                    active = false;
-                } else if (k >= kmax) {
-                    st = ENS_DONE_STEPS;
-                    active = false;
-                }
-            }
         }
-        // lanes that just stopped take no part in the shuffles below: re-vote (every lane of amask is here)
+    };
+    // predict: the step is now certain to be taken, so its bookkeeping (time, step count) is done here, a whole step
+    // ahead of the quick test that reads it.  am2 = the lanes that take the step.
+    auto predict = [&](unsigned am2) {
+        double p_a = p.p_a, p_j = p.p_j, cx_a = p.cx_a, cx_j = p.cx_j, cv_a = p.cv_a, cv_j = p.cv_j;
+        if constexpr (ADAPT) {
+            h = adaptive_dt<N, L, B>(a, j, p.dt, l, base, am2);
+            const double h2 = h * h, h3 = h2 * h;
+            p_a = 0.5 * h2;
+            p_j = (1.0 / 6.0) * h3;
+            cx_a = 0.35 * h2;
+            cx_j = 0.05 * h3;
+            cv_a = 0.5 * h;
+            cv_j = (1.0 / 12.0) * h2;
+        }
+        if constexpr (UNROLL) {  // (the 3-phase loop does it in its last phase: fewer values live across the evaluations)
+            ts += fabs(h);       // h carries the sign of the direction
+            ++k;
+        }
+#pragma unroll
+        for (int b = 0; b < B; ++b)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double tx = fma(h, V[b][c], X[b][c]);
+                Cx[b][c] = fma(cx_j, j[b][c], fma(cx_a, a[b][c], tx));
+                Cv[b][c] = fma(cv_j, j[b][c], fma(cv_a, a[b][c], V[b][c]));
+                X[b][c] = fma(p_j, j[b][c], fma(p_a, a[b][c], tx));
+                V[b][c] = fma(p_a, j[b][c], fma(h, a[b][c], V[b][c]));
+            }
+    };
+    auto accept_and_predict = [&](unsigned amask) {
+        if (__builtin_expect(quick_test(amask) != 0u, 0)) exact_stop(amask);
+        // lanes that just stopped take no part in the shuffles of predict: re-vote (every lane of amask is here)
         unsigned am2 = amask;
         if constexpr (ADAPT && L > 1) am2 = __ballot_sync(amask, active);
-        if (active) {
-            double p_a = p.p_a, p_j = p.p_j, cx_a = p.cx_a, cx_j = p.cx_j, cv_a = p.cv_a, cv_j = p.cv_j;
-            if constexpr (ADAPT) {
-                h = adaptive_dt<N, L, B>(a, j, p.dt, l, base, am2);
-                const double h2 = h * h, h3 = h2 * h;
-                p_a = 0.5 * h2;
-                p_j = (1.0 / 6.0) * h3;
-                cx_a = 0.35 * h2;
-                cx_j = 0.05 * h3;
-                cv_a = 0.5 * h;
-                cv_j = (1.0 / 12.0) * h2;
-            }
-#pragma unroll
-            for (int b = 0; b < B; ++b)
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    const double tx = fma(h, V[b][c], X[b][c]);
-                    Cx[b][c] = fma(cx_j, j[b][c], fma(cx_a, a[b][c], tx));
-                    Cv[b][c] = fma(cv_j, j[b][c], fma(cv_a, a[b][c], V[b][c]));
-                    X[b][c] = fma(p_j, j[b][c], fma(p_a, a[b][c], tx));
-                    V[b][c] = fma(p_a, j[b][c], fma(h, a[b][c], V[b][c]));
-                }
-        }
+        if (active) predict(am2);
     };
     auto correct = [&]() {
         double kx_a = p.kx_a, kx_j = p.kx_j, kv_a = p.kv_a, kv_j = p.kv_j;
@@ -486,7 +496,32 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
 
     bool fresh = true;  // CARRY: a, j do not yet belong to the current state (warp-uniform: start of the launch)
     auto run = [&]() {
-    if constexpr (UNROLL) {
+    if constexpr (UNROLL && !ADAPT) {
+        // Straight-line step, fixed step size: the systems of the warp that run enter the loop together (mask am) and
+        // stay in it until the exact stop logic retires them; it runs only when the quick test fails for some lane, so a
+        // step costs one vote, one almost never taken branch and the loop's jump.
+        const unsigned amask0 = __ballot_sync(0xffffffffu, active);
+        if (active) {
+            unsigned am = amask0;
+            while (true) {
+                if (!CARRY || fresh)
+                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, am);
+                else
+                    r2min = p.rc2_bits ? (unsigned)(pair_r2min<N, L, B>(X, l, base, am) >> 32) : ~0u;
+                fresh = false;
+                if (__builtin_expect(quick_test(am) != 0u, 0)) {
+                    exact_stop(am);
+                    am = __ballot_sync(am, active);  // the lanes that go on
+                    if (!active) break;
+                }
+                predict(am);
+                eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am);
+                correct();
+                eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am);
+                correct();
+            }
+        }
+    } else if constexpr (UNROLL) {
         while (true) {
             if constexpr (ADAPT) {
                 if (!refill()) break;
@@ -510,8 +545,6 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                     correct();
                     eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am2);
                     correct();
-                    ts += fabs(h);  // h carries the sign of the direction
-                    ++k;
                 }
             }
             fresh = false;
@@ -540,7 +573,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 } else {
                     correct();
                     if (phase == 2) {
-                        ts += fabs(h);  // h carries the sign of the direction
+                        ts += fabs(h);
                         ++k;
                     }
                 }
