@@ -763,7 +763,7 @@ int ens_get_info(const ens_t* e, int64_t out[10]) {
         out[5] = fa.numRegs;
         out[8] = (int64_t)fa.localSizeBytes;
         int nb = 0;
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, ki->fn, threads, 0));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, ki->fn, threads, (size_t)(threads / 32) * ki->smem_bytes_per_warp));
         out[6] = nb;
     }
     out[7] = e->launches;

@@ -76,6 +76,7 @@ struct KernelInfo {
     const void* fn;
     Shape shape;
     int threads;  // threads per block
+    int smem_bytes_per_warp = 0;  // dynamic shared memory the kernel is launched with, per warp of the block
 };
 
 // Launch-time choices a test or a measurement may override through ens_test_set_option (0 = the library's default).

@@ -75,7 +75,15 @@ KernelInfo info_of() {
     k.shape.L = S::L;
     k.shape.B = S::B;
     k.threads = S::THREADS;
+    k.smem_bytes_per_warp = ring_smem_words<S::L, S::B>() * (int)sizeof(double2);
     return k;
+}
+
+// dynamic shared memory of a block of `threads` threads (the cross-lane ring's visitor and return words; 0 for L = 1)
+template <int N, int MODE>
+constexpr size_t ring_smem_bytes(int threads) {
+    using S = ShapeOf<N, MODE>;
+    return (size_t)(threads / 32) * ring_smem_words<S::L, S::B>() * sizeof(double2);
 }
 
 // blocks of `threads` threads the device holds at once
@@ -84,7 +92,7 @@ cudaError_t resident_blocks(int threads, int64_t* out) {
     int dev = 0, sms = 0, per_sm = 0;
     cudaError_t err = cudaGetDevice(&dev);
     if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel_ptr<N, MODE>(), threads, 0);
+    if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel_ptr<N, MODE>(), threads, ring_smem_bytes<N, MODE>(threads));
     *out = (int64_t)sms * (per_sm > 0 ? per_sm : 1);
     return err;
 }
@@ -140,13 +148,13 @@ cudaError_t launch_n(const View& v, StepArgs a, const LaunchTune& tune, cudaStre
             if ((err = cudaMemsetAsync(a.slice_done, 0, sizeof(int32_t) * (size_t)warps, s)) != cudaSuccess) return err;
             if (blocks_out) *blocks_out = blocks;
             if (fn_out) *fn_out = (const void*)kernel_ptr<N, 3>();
-            kernel_ptr<N, 3>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
+            kernel_ptr<N, 3>()<<<(unsigned)blocks, threads, ring_smem_bytes<N, 3>(threads), s>>>(v, a);
             return cudaGetLastError();
         }
     }
     if (blocks_out) *blocks_out = blocks;
     if (fn_out) *fn_out = (const void*)kernel_ptr<N, MODE>();
-    kernel_ptr<N, MODE>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
+    kernel_ptr<N, MODE>()<<<(unsigned)blocks, threads, ring_smem_bytes<N, MODE>(threads), s>>>(v, a);
     return cudaGetLastError();
 }
 

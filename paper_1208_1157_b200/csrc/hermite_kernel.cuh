@@ -62,47 +62,70 @@ __device__ __forceinline__ double pair_acc_jerk(const double (&xi)[3], const dou
     return r2;
 }
 
+// Shared memory of the cross-lane schedule (L > 1 only), per warp, in 16-byte words laid out word-major (word w of lane
+// n at [w * 32 + n]: a warp's access touches every bank group once per quarter warp unless two systems of the quarter
+// straddle it):
+//   visitors  B * 4 words per lane: (x0, x1) (x2, v0) (v1, v2) (m, -) of each of the lane's bodies
+//   returns   2 * 3 words per lane: (a0, a1) (a2, j0) (j1, j2), double-buffered over the visits (RET_SMEM shapes)
+template <int L, int B>
+__host__ __device__ constexpr int ring_smem_words() {
+    return L > 1 ? B * 4 * 32 + 6 * 32 : 0;
+}
+// which shapes send the returned halves through shared memory instead of shuffles (measured, DESIGN.md section 8:
+// a gain for 5 lanes x 3 bodies, a loss for the shapes with 2 bodies per lane, neutral for 3 lanes)
+template <int L, int B>
+__host__ __device__ constexpr bool ring_returns_in_smem() {
+    return L == 5 && B == 3;
+}
+
 // Acceleration and jerk of the B bodies this lane owns, every pair of the system once.
-// l = lane index inside the system (0..L-1), base = first lane of the system in the warp, amask = active lanes.
+// l = lane index inside the system (0..L-1), base = first lane of the system in the warp, amask = active lanes,
+// W = this warp's shared memory (ring_smem_words; unused for L = 1).
 // TRACK = false skips the minimum pair distance (only a step's first evaluation feeds the monitor).  The minimum is
 // kept as the smallest HIGH WORD of the squared separations' bit patterns (one integer min per pair, off the FP64
 // pipe); monitor_flags decides exactly from it, recomputing the full 64-bit minimum only in the rare tie.
 template <int N, int L, int B, bool TRACK = true>
 __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const double (&v)[B][3], const double (&m)[B],
                                               double (&a)[B][3], double (&j)[B][3], unsigned& r2min, int l, int base,
-                                              unsigned amask) {
+                                              unsigned amask, double2* W) {
     constexpr bool PADDED = (L * B != N);
+    constexpr bool RET_SMEM = ring_returns_in_smem<L, B>();
 #pragma unroll
     for (int b = 0; b < B; ++b)
 #pragma unroll
         for (int c = 0; c < 3; ++c) a[b][c] = j[b][c] = 0.0;
     if constexpr (TRACK) r2min = ~0u;
 
-    // Cross-lane schedule (L > 1), written so that shuffle latency hides behind FP64 work of the same warp (a warp
-    // issues in order: an instruction that waits on a shuffle blocks everything behind it) and so that few values are
-    // live at once (the visitors of the next shift arrive body by body while those of the current one are used up, and
-    // the returned halves are added one body behind):
-    //   fetch(shift 1) | in-lane pairs among bodies 1.. |
-    //   for s = 1..H, for each visitor body c: { fetch body c of shift s+1 | B pairs (my bodies x visitor c) |
+    // Cross-lane schedule (L > 1): every lane publishes its bodies in shared memory (four 16-byte stores per body,
+    // two warp barriers per evaluation) and reads the visiting body right before the pairs that use it (four 16-byte
+    // loads instead of the 14 shuffles and the double-buffered visitor registers of the earlier shuffle ring):
+    //   publish | in-lane pairs among bodies 1.. |
+    //   for s = 1..H, for each visitor body c: { read body c of lane l + s | B pairs (my bodies x visitor c) |
     //                                            add the returns for my body c-1 | send the returns for visitor c } |
     //   in-lane pairs with body 0 | add the last returns
+    // The returned halves (Newton's third law: the visitor's share of the B pairs) travel by shuffle, or through the
+    // owner's shared-memory slot where that is faster (RET_SMEM), and are added one visit behind.
     constexpr int H = (L - 1) / 2;
-    double xv[2][B][3], vv[2][B][3], mv[2][B];  // visitors, double-buffered over the shifts
-    auto fetch_body = [&](int s, int c, int buf) {
-        int ls = l + s;
-        if (ls >= L) ls -= L;
-        const int src = base + ls;  // whose bodies visit this lane at shift s
-#pragma unroll
-        for (int q = 0; q < 3; ++q) {
-            xv[buf][c][q] = __shfl_sync(amask, x[c][q], src);
-            vv[buf][c][q] = __shfl_sync(amask, v[c][q], src);
-        }
-        mv[buf][c] = __shfl_sync(amask, m[c], src);
-    };
+    const int wl = threadIdx.x & 31;
     if constexpr (L > 1) {
+        __syncwarp(amask);  // every lane has finished reading the previous publication
 #pragma unroll
-        for (int c = 0; c < B; ++c) fetch_body(1, c, 1);
+        for (int c = 0; c < B; ++c) {
+            W[(c * 4 + 0) * 32 + wl] = make_double2(x[c][0], x[c][1]);
+            W[(c * 4 + 1) * 32 + wl] = make_double2(x[c][2], v[c][0]);
+            W[(c * 4 + 2) * 32 + wl] = make_double2(v[c][1], v[c][2]);
+            W[(c * 4 + 3) * 32 + wl] = make_double2(m[c], 0.0);
+        }
+        __syncwarp(amask);
     }
+    double xv[3], vv[3], mv;  // the visiting body
+    auto fetch_body = [&](int src, int c) {
+        const double2 w0 = W[(c * 4 + 0) * 32 + src], w1 = W[(c * 4 + 1) * 32 + src], w2 = W[(c * 4 + 2) * 32 + src],
+                      w3 = W[(c * 4 + 3) * 32 + src];
+        xv[0] = w0.x, xv[1] = w0.y, xv[2] = w1.x;
+        vv[0] = w1.y, vv[1] = w2.x, vv[2] = w2.y;
+        mv = w3.x;
+    };
 
     // pairs inside the lane.  Order: pairs among bodies 1.. first, pairs with local body 0 last, so that on lane 0
     // every planet receives the star's (largest) contribution last (for L = 1 this is exactly the
@@ -118,8 +141,15 @@ __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const dou
     for (int b = 1; b < B; ++b) in_lane(b);
 
     if constexpr (L > 1) {
-        double ra[3], rj[3];  // the other half of the pairs of ONE of my bodies, computed by lane l - s; in flight
-        auto add_returns = [&](int body) {
+        double2* const R = W + B * 4 * 32;  // return slots
+        double ra[3], rj[3];                // shuffle path: the other half of the pairs of ONE of my bodies, in flight
+        auto add_returns = [&](int body, int slot) {
+            if constexpr (RET_SMEM) {
+                const double2 r0 = R[(slot * 3 + 0) * 32 + wl], r1 = R[(slot * 3 + 1) * 32 + wl],
+                              r2 = R[(slot * 3 + 2) * 32 + wl];
+                ra[0] = r0.x, ra[1] = r0.y, ra[2] = r1.x;
+                rj[0] = r1.y, rj[1] = r2.x, rj[2] = r2.y;
+            }
 #pragma unroll
             for (int q = 0; q < 3; ++q) {
                 a[body][q] += ra[q];
@@ -128,36 +158,43 @@ __device__ __forceinline__ void eval_acc_jerk(const double (&x)[B][3], const dou
         };
 #pragma unroll
         for (int s = 1; s <= H; ++s) {
-            const int buf = s & 1;
-            int ls = l + s;
+            int ls = l + s;  // whose bodies visit this lane at shift s: it owns the halves computed here
             if (ls >= L) ls -= L;
-            int lr = l - s;
+            int lr = l - s;  // the lane this lane's bodies visit: it computes the halves this lane gets back
             if (lr < 0) lr += L;
-            const int ret = base + lr;
 #pragma unroll
             for (int c = 0; c < B; ++c) {
-                if (s < H) fetch_body(s + 1, c, buf ^ 1);
+                const int vis = (s - 1) * B + c;
+                fetch_body(base + ls, c);
                 double av[3], jv[3];  // the visitor's half of these B pairs: started by the first pair
                 const bool vvalid = !PADDED || (ls * B + c < N);
 #pragma unroll
                 for (int b = 0; b < B; ++b) {
-                    const double r2 = b == 0 ? pair_acc_jerk<true>(x[b], v[b], m[b], a[b], j[b], xv[buf][c], vv[buf][c],
-                                                                   mv[buf][c], av, jv)
-                                             : pair_acc_jerk(x[b], v[b], m[b], a[b], j[b], xv[buf][c], vv[buf][c],
-                                                             mv[buf][c], av, jv);
+                    const double r2 = b == 0 ? pair_acc_jerk<true>(x[b], v[b], m[b], a[b], j[b], xv, vv, mv, av, jv)
+                                             : pair_acc_jerk(x[b], v[b], m[b], a[b], j[b], xv, vv, mv, av, jv);
                     if constexpr (TRACK) min_hi(r2min, r2, vvalid && (!PADDED || (l * B + b < N)));
                 }
-                if (c > 0) add_returns(c - 1);  // sent one visitor body ago
-                else if (s > 1) add_returns(B - 1);
+                if constexpr (RET_SMEM) {
+                    if (vis >= 1) {
+                        __syncwarp(amask);  // the returns of the previous visit are written (and its slot's last reads done)
+                        add_returns((vis - 1) % B, (vis - 1) & 1);
+                    }
+                    R[((vis & 1) * 3 + 0) * 32 + base + ls] = make_double2(av[0], av[1]);
+                    R[((vis & 1) * 3 + 1) * 32 + base + ls] = make_double2(av[2], jv[0]);
+                    R[((vis & 1) * 3 + 2) * 32 + base + ls] = make_double2(jv[1], jv[2]);
+                } else {
+                    if (vis >= 1) add_returns((vis - 1) % B, 0);  // sent one visit ago
 #pragma unroll
-                for (int q = 0; q < 3; ++q) {
-                    ra[q] = __shfl_sync(amask, av[q], ret);
-                    rj[q] = __shfl_sync(amask, jv[q], ret);
+                    for (int q = 0; q < 3; ++q) {
+                        ra[q] = __shfl_sync(amask, av[q], base + lr);
+                        rj[q] = __shfl_sync(amask, jv[q], base + lr);
+                    }
                 }
             }
         }
         in_lane(0);
-        add_returns(B - 1);
+        if constexpr (RET_SMEM) __syncwarp(amask);
+        add_returns(B - 1, (H * B - 1) & 1);
     } else {
         in_lane(0);
     }
@@ -290,6 +327,8 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
     constexpr bool PADDED = (L * B != N);
     const int lane = threadIdx.x & 31;
     const int64_t warp = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    extern __shared__ double2 ring_smem[];  // ring_smem_words<L, B>() per warp (nothing for L = 1)
+    double2* const W = ring_smem + (threadIdx.x >> 5) * ring_smem_words<L, B>();
     const int sl = lane / L;
     const int l = lane - sl * L;
     const int base = sl * L;
@@ -505,7 +544,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
             unsigned am = amask0;
             while (true) {
                 if (!CARRY || fresh)
-                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, am);
+                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, am, W);
                 else
                     r2min = p.rc2_bits ? (unsigned)(pair_r2min<N, L, B>(X, l, base, am) >> 32) : ~0u;
                 fresh = false;
@@ -515,9 +554,9 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                     if (!active) break;
                 }
                 predict(am);
-                eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am);
+                eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am, W);
                 correct();
-                eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am);
+                eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am, W);
                 correct();
             }
         }
@@ -533,7 +572,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
             }
             if (active) {
                 if (!CARRY || fresh)
-                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
+                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask, W);
                 else
                     r2min = p.rc2_bits ? (unsigned)(pair_r2min<N, L, B>(X, l, base, amask) >> 32) : ~0u;
                 accept_and_predict(amask);
@@ -541,9 +580,9 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 unsigned am2 = amask;
                 if constexpr (L > 1) am2 = __ballot_sync(amask, active);
                 if (active) {
-                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am2);
+                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am2, W);
                     correct();
-                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am2);
+                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am2, W);
                     correct();
                 }
             }
@@ -565,7 +604,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
             }
             if (active) {
                 if (!CARRY || fresh || phase != 0)
-                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask);
+                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask, W);
                 else
                     r2min = p.rc2_bits ? (unsigned)(pair_r2min<N, L, B>(X, l, base, amask) >> 32) : ~0u;
                 if (phase == 0) {
