@@ -45,6 +45,7 @@ KernelInfo info_of() {
     k.shape.L = S::L;
     k.shape.B = S::B;
     k.threads = S::THREADS;
+    k.smem_bytes_per_warp = acc_ring_smem_words<S::L, S::B>() * (int)sizeof(double2);
     return k;
 }
 
@@ -57,7 +58,7 @@ cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t
     const int wpb = threads / 32;
     const int64_t blocks = (warps + wpb - 1) / wpb;
     if (blocks_out) *blocks_out = blocks;
-    kernel_ptr<N, MERGED>()<<<(unsigned)blocks, threads, 0, s>>>(v, a);
+    kernel_ptr<N, MERGED>()<<<(unsigned)blocks, threads, (size_t)(threads / 32) * acc_ring_smem_words<S::L, S::B>() * sizeof(double2), s>>>(v, a);
     return cudaGetLastError();
 }
 

@@ -310,6 +310,8 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
     const int base = sl * L;
     const int64_t sys = warp * S + sl;
     const bool live = (sl < S) && (sys < e.n_sys);
+    extern __shared__ double2 ring_smem[];  // acc_ring_smem_words<L, B>() per warp (nothing for L = 1)
+    double2* const W = ring_smem + (threadIdx.x >> 5) * acc_ring_smem_words<L, B>();
 
     double Q[B][3], V[B][3], A[B][3], m[B];
     double Xcm[3] = {0.0, 0.0, 0.0}, Vcm[3] = {0.0, 0.0, 0.0};
@@ -389,7 +391,7 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
     {  // prepare(P) (Alg. 1): accelerations and drift velocity of the initial state
         const unsigned amask = __ballot_sync(0xffffffffu, active);
         if (active) {
-            eval_acc_planets<P, L, B>(Q, m, A, r2min, l, base, amask);
+            eval_acc_planets<P, L, B>(Q, m, A, r2min, l, base, amask, W);
             mass_weighted_sum<L, B>(V, m, s, l, base, amask);
 #pragma unroll
             for (int c = 0; c < 3; ++c) s[c] = s[c] * im0;
@@ -443,7 +445,7 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
                 for (int c = 0; c < 3; ++c) s[c] = s[c] * im0;
             }
             // 4: planet-planet accelerations at the new positions, half kick
-            eval_acc_planets<P, L, B>(Q, m, A, r2min, l, base, am);
+            eval_acc_planets<P, L, B>(Q, m, A, r2min, l, base, am, W);
             if constexpr (!MERGED) {
 #pragma unroll
                 for (int b = 0; b < B; ++b)

@@ -53,6 +53,7 @@ KernelInfo info_of() {
     k.shape.L = S::L;
     k.shape.B = S::B;
     k.threads = S::THREADS;
+    k.smem_bytes_per_warp = acc_ring_smem_words<S::L, S::B>() * (int)sizeof(double2);
     return k;
 }
 
@@ -135,12 +136,12 @@ cudaError_t launch_adaptive_n(const View& v, const StepArgs& a, int threads, cud
     int dev = 0, sms = 0, per_sm = 0;  // persistent grid: what the device holds at once
     cudaError_t err = cudaGetDevice(&dev);
     if (err == cudaSuccess) err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel_ptr<N, true>(), threads, 0);
+    if (err == cudaSuccess) err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel_ptr<N, true>(), threads, (size_t)(threads / 32) * acc_ring_smem_words<S::L, S::B>() * sizeof(double2));
     if (err != cudaSuccess) return err;
     const int64_t resident = (int64_t)sms * (per_sm > 0 ? per_sm : 1);
     if (blocks > resident) blocks = resident;
     if (blocks_out) *blocks_out = blocks;
-    kernel_ptr<N, true>()<<<(unsigned)blocks, threads, 0, s>>>(v, a, unit_coefficients());
+    kernel_ptr<N, true>()<<<(unsigned)blocks, threads, (size_t)(threads / 32) * acc_ring_smem_words<S::L, S::B>() * sizeof(double2), s>>>(v, a, unit_coefficients());
     return cudaGetLastError();
 }
 
@@ -153,7 +154,7 @@ cudaError_t launch_n(const View& v, const StepArgs& a, int threads, cudaStream_t
     const int wpb = threads / 32;
     const int64_t blocks = (warps + wpb - 1) / wpb;
     if (blocks_out) *blocks_out = blocks;
-    kernel_ptr<N>()<<<(unsigned)blocks, threads, 0, s>>>(v, a, coefficients(a.dt));
+    kernel_ptr<N>()<<<(unsigned)blocks, threads, (size_t)(threads / 32) * acc_ring_smem_words<S::L, S::B>() * sizeof(double2), s>>>(v, a, coefficients(a.dt));
     return cudaGetLastError();
 }
 

@@ -38,6 +38,8 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
     const int base = sl * L;
     const int64_t sys = warp * S + sl;
     const bool live = (sl < S) && (sys < e.n_sys);
+    extern __shared__ double2 ring_smem[];  // acc_ring_smem_words<L, B>() per warp (nothing for L = 1)
+    double2* const W = ring_smem + (threadIdx.x >> 5) * acc_ring_smem_words<L, B>();
 
     double X[B][3], V[B][3], m[B];
     // time folded with the direction of the run (ts = t forward, -t backward: exact), end test ts < p.te either way
@@ -81,7 +83,7 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
         if (amask == 0) break;
         if (active) {
             // stage 1 at the accepted state: also the monitors' pair distances (Alg. 1: advance, then execute(M))
-            eval_acc_planets<N, L, B>(X, m, K[0], r2min, l, base, amask);
+            eval_acc_planets<N, L, B>(X, m, K[0], r2min, l, base, amask, W);
             // One quick test per step (as in hermite_kernel.cuh): every pair this lane saw farther apart than r_close and
             // every coordinate of its bodies below r_eject / sqrt(3), both on high words (the exact decisions cannot
             // differ; non-finite values fail it), time left, steps left.  The exact monitor / stop logic runs only when
@@ -146,9 +148,9 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
                             Xs[b][c] = s;
                         }
                     if (i < 5)
-                        eval_acc_planets<N, L, B>(Xs, m, K[i], dummy, l, base, am2);
+                        eval_acc_planets<N, L, B>(Xs, m, K[i], dummy, l, base, am2, W);
                     else
-                        eval_acc_planets<N, L, B>(Xs, m, K6, dummy, l, base, am2);
+                        eval_acc_planets<N, L, B>(Xs, m, K6, dummy, l, base, am2, W);
                 }
 #pragma unroll
                 for (int b = 0; b < B; ++b)
@@ -232,6 +234,8 @@ __global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkU
     const int l = lane - sl * L;
     const int base = sl * L;
     int64_t sys = 0;
+    extern __shared__ double2 ring_smem[];  // acc_ring_smem_words<L, B>() per warp (nothing for L = 1)
+    double2* const W = ring_smem + (threadIdx.x >> 5) * acc_ring_smem_words<L, B>();
 
     double X[B][3], V[B][3], m[B];
     double t = 0.0, h = p.dt;
@@ -334,7 +338,7 @@ __global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkU
             // pair distances (Alg. 1: advance, then execute(M)) and the loop tests.  A rejected trial skips all this.
             const unsigned kmask = __ballot_sync(amask, !have_k1);  // the lanes that take stage 1 (and its quick test)
             if (!have_k1) {
-                eval_acc_planets<N, L, B>(X, m, K[0], r2min, l, base, kmask);
+                eval_acc_planets<N, L, B>(X, m, K[0], r2min, l, base, kmask, W);
                 have_k1 = true;
                 // the quick test of the fixed-step kernel; the exact logic only when some lane of kmask fails it
                 unsigned cmax = 0u;
@@ -396,9 +400,9 @@ __global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkU
                             Xs[b][c] = fma(h2, s, fma(ch, V[b][c], X[b][c]));
                         }
                     if (i < 5)
-                        eval_acc_planets<N, L, B>(Xs, m, K[i], dummy, l, base, am2);
+                        eval_acc_planets<N, L, B>(Xs, m, K[i], dummy, l, base, am2, W);
                     else
-                        eval_acc_planets<N, L, B>(Xs, m, K6, dummy, l, base, am2);
+                        eval_acc_planets<N, L, B>(Xs, m, K6, dummy, l, base, am2, W);
                 }
                 // error level of this trial (scales from the state the step starts from)
                 double ex = 0.0, ev = 0.0, x2 = 0.0, v2 = 0.0;
