@@ -561,32 +561,28 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
             }
         }
     } else if constexpr (UNROLL) {
-        while (true) {
-            if constexpr (ADAPT) {
-                if (!refill()) break;
-            }
+        // Straight-line step, adaptive step size (persistent grid).  The groups that hold a system run the same inner
+        // loop as above; when the exact stop logic retires a system the whole warp leaves it (a warp-uniform break), so
+        // that the idle group pulls its next system at this step boundary.  The groups that go on re-enter and repeat
+        // the evaluation they had just done (same state, same result, bit for bit): one evaluation per retirement
+        // and warp, about 0.5 % of the work of a launch.
+        while (refill()) {
             const unsigned amask = __ballot_sync(0xffffffffu, active);
-            if (amask == 0) {
-                if constexpr (ADAPT) continue;
-                break;
-            }
+            if (amask == 0) continue;
             if (active) {
-                if (!CARRY || fresh)
+                while (true) {
                     eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, amask, W);
-                else
-                    r2min = p.rc2_bits ? (unsigned)(pair_r2min<N, L, B>(X, l, base, amask) >> 32) : ~0u;
-                accept_and_predict(amask);
-                // lanes that just stopped take no part in the shuffles of the corrector evaluations
-                unsigned am2 = amask;
-                if constexpr (L > 1) am2 = __ballot_sync(amask, active);
-                if (active) {
-                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am2, W);
+                    if (__builtin_expect(quick_test(amask) != 0u, 0)) {
+                        exact_stop(amask);
+                        if (__ballot_sync(amask, active) != amask) break;  // some group retired its system
+                    }
+                    predict(amask);
+                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, amask, W);
                     correct();
-                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am2, W);
+                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, amask, W);
                     correct();
                 }
             }
-            fresh = false;
         }
     } else {
         int phase = 0;  // warp-uniform: 0 = accept + predict, 1 and 2 = corrector iterations
