@@ -78,10 +78,11 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
     double K[5][B][3];  // stage accelerations k_1 .. k_5
     u64 r2min;
 
-    while (true) {
-        const unsigned amask = __ballot_sync(0xffffffffu, active);
-        if (amask == 0) break;
-        if (active) {
+    // The systems of the warp that run enter the loop together (mask amask) and stay in it until the exact stop logic
+    // retires them (hermite_kernel.cuh): one vote and one almost never taken branch per step.
+    unsigned amask = __ballot_sync(0xffffffffu, active);
+    if (active) {
+        while (true) {
             // stage 1 at the accepted state: also the monitors' pair distances (Alg. 1: advance, then execute(M))
             eval_acc_planets<N, L, B>(X, m, K[0], r2min, l, base, amask, W);
             // One quick test per step (as in hermite_kernel.cuh): every pair this lane saw farther apart than r_close and
@@ -129,11 +130,11 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
                         active = false;
                     }
                 }
+                amask = __ballot_sync(amask, active);  // the lanes that go on
+                if (!active) break;
             }
-            // lanes that just stopped take no part in the shuffles of the remaining stages
-            unsigned am2 = amask;
-            if constexpr (L > 1) am2 = __ballot_sync(amask, active);
-            if (active) {
+            {
+                const unsigned am2 = amask;
                 double Xs[B][3], K6[B][3];
                 u64 dummy;
 #pragma unroll
