@@ -36,11 +36,12 @@ __constant__ double kStumpff[16] = {
 
 __device__ __forceinline__ void stumpff_series(double z, double& c0, double& c1, double& c2, double& c3) {
     // Horner in z; the coefficients are constant-bank operands of the DFMAs (no registers, no immediates to build)
-    // the z^7 coefficients (-1/16!, -1/17!) truncated to their high words: built with one move each instead of a
-    // constant load the first DFMA would have to wait for; their term is < 5e-21, its truncation error < 3e-27
-    double s2 = -0x1.ae7f3p-45, s3 = -0x1.952c7p-49;
+    // the z^7 and z^6 coefficients (-1/16!, -1/17!, 1/14!, 1/15!) truncated to their high words: literals built with one
+    // move each, so that the first DFMA does not wait for a constant load (a DFMA takes one constant-bank operand);
+    // their terms are < 5e-21 and < 1.2e-17, the truncation errors < 3e-27 and < 6e-24
+    double s2 = fma(-0x1.ae7f3p-45, z, 0x1.93974p-37), s3 = fma(-0x1.952c7p-49, z, 0x1.ae7f3p-41);
 #pragma unroll
-    for (int k = 1; k < 8; ++k) {
+    for (int k = 2; k < 8; ++k) {
         s2 = fma(s2, z, kStumpff[2 * k]);
         s3 = fma(s3, z, kStumpff[2 * k + 1]);
     }
