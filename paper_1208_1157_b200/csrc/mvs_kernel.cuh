@@ -25,8 +25,8 @@
 
 namespace ensd {
 
-// Stumpff functions c_n(z) = sum_k (-z)^k / (2k+n)!  (R-M3), series part: valid for |z| <= 0.1 (8 terms: truncation
-// < 1e-21 relative).  For the step sizes of the workloads (h << orbital period) z = beta X^2 is always in this range.
+// Stumpff functions c_n(z) = sum_k (-z)^k / (2k+n)!  (R-M3), series part: valid for |z| <= 0.1 (7 terms: truncation
+// < 1e-20 relative).  For the step sizes of the workloads (h << orbital period) z = beta X^2 is always in this range.
 __constant__ double kStumpff[16] = {
     // descending powers of z, c2 / c3 interleaved: -1/16!, -1/17!, 1/14!, 1/15!, ..., 1/2!, 1/3!
     -1.0 / 20922789888000.0, -1.0 / 355687428096000.0, 1.0 / 87178291200.0, 1.0 / 1307674368000.0,
@@ -36,10 +36,11 @@ __constant__ double kStumpff[16] = {
 
 __device__ __forceinline__ void stumpff_series(double z, double& c0, double& c1, double& c2, double& c3) {
     // Horner in z; the coefficients are constant-bank operands of the DFMAs (no registers, no immediates to build)
-    // the z^7 and z^6 coefficients (-1/16!, -1/17!, 1/14!, 1/15!) truncated to their high words: literals built with one
-    // move each, so that the first DFMA does not wait for a constant load (a DFMA takes one constant-bank operand);
-    // their terms are < 5e-21 and < 1.2e-17, the truncation errors < 3e-27 and < 6e-24
-    double s2 = fma(-0x1.ae7f3p-45, z, 0x1.93974p-37), s3 = fma(-0x1.952c7p-49, z, 0x1.ae7f3p-41);
+    // Seven terms (up to z^6): for |z| <= 0.1 the z^7 terms are < 5e-21 of c2 = 1/2, c3 = 1/6.  The leading (z^6)
+    // coefficients 1/14!, 1/15! are literals truncated to their high words (their terms are < 1.2e-17, the truncation
+    // error < 6e-24): built with one move each, so that the first DFMA does not wait for a constant load (a DFMA takes
+    // one constant-bank operand).
+    double s2 = 0x1.93974p-37, s3 = 0x1.ae7f3p-41;
 #pragma unroll
     for (int k = 2; k < 8; ++k) {
         s2 = fma(s2, z, kStumpff[2 * k]);
