@@ -149,39 +149,40 @@ constexpr int kHiConv2 = 0x3db00000;  // high word of kConv^2 = 2^-36
 //   * Stumpff arguments beyond the series range (|z| > 0.1: steps of a sizeable fraction of a period) and lanes
 //     that fail to converge within the cap take out-of-line general paths.
 // valid(b) = false leaves slot b untouched (massless dummy slots of padded shapes).
-template <int B, class Valid>
-__device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[B][3], double mu, double tau,
-                                                 unsigned amask, Valid valid) {
+// Fourth-order series start of the universal Kepler equation (see kepler_drift_all); returns the correction `corr`
+// with X = u (1 + corr).
+__device__ __forceinline__ double kepler_series_start(double u, double ir0, double r0, double eta, double beta, double mu) {
+    const double e1 = eta * ir0, e2 = e1 * e1, br = beta * r0;
+    const double k = mu - br;
+    const double q3 = fma(-1.0 / 6.0, k * ir0, 0.5 * e2);
+    const double q4 = fma(-0.625, e2 * e1, (e1 * ir0) * fma(1.0 / 24.0, br, (5.0 / 12.0) * k));
+    return u * fma(u, fma(u, q4, q3), -0.5 * e1);
+}
+
+// The general procedure of the Kepler drift (R-M4), for the lanes the fast path of kepler_drift_all does not stand for:
+// all B planets of the lane from the start.  Out of line (the state goes through local memory): rarely called.
+template <int B>
+struct KeplerLane {
     double r0[B], ir0[B], eta[B], beta[B], X[B], d[B];
     KeplerG g[B];
+};
+template <int B>
+__device__ __noinline__ void kepler_general_solve(KeplerLane<B>& s, double mu, double tau) {
+    double(&r0)[B] = s.r0;
+    double(&ir0)[B] = s.ir0;
+    double(&eta)[B] = s.eta;
+    double(&beta)[B] = s.beta;
+    double(&X)[B] = s.X;
+    double(&d)[B] = s.d;
+    KeplerG(&g)[B] = s.g;
+    int ok[B];
 #pragma unroll
     for (int b = 0; b < B; ++b) {
-        const double r02 = fma(Q[b][2], Q[b][2], fma(Q[b][1], Q[b][1], Q[b][0] * Q[b][0]));
-        eta[b] = fma(Q[b][2], P[b][2], fma(Q[b][1], P[b][1], Q[b][0] * P[b][0]));
-        const double v2 = fma(P[b][2], P[b][2], fma(P[b][1], P[b][1], P[b][0] * P[b][0]));
-        ir0[b] = rsqrt_f64(r02);
-        r0[b] = r02 * ir0[b];
-        beta[b] = fma(2.0 * mu, ir0[b], -v2);
-        // Starting value: the universal Kepler equation is the power series
-        //   tau = r0 X + eta X^2 / 2 + (mu - beta r0) X^3 / 6 - beta eta X^4 / 24 + ...
-        // and its reversion to fourth order in u = tau / r0,
-        //   X = u (1 + u (q2 + u (q3 + u q4))),   q2 = -e1 / 2,  q3 = e1^2 / 2 - k / (6 r0),
-        //   q4 = e1 (5 k / 12 + beta r0 / 24) / r0 - 5 e1^3 / 8,   e1 = eta / r0,  k = mu - beta r0,
-        // is within 1e-6 of the root for steps of a few per cent of a period (config 4: max 7e-7), so that ONE
-        // Chebyshev step reaches rounding level; the plain guess X = u (the oracle's, R-M4) needs two.  Same root.
-        // Steps too long for the series (correction not small) start from X = u.
         const double u = tau * ir0[b];
-        const double e1 = eta[b] * ir0[b], e2 = e1 * e1, br = beta[b] * r0[b];
-        const double k = mu - br;
-        const double q3 = fma(-1.0 / 6.0, k * ir0[b], 0.5 * e2);
-        const double q4 = fma(-0.625, e2 * e1, (e1 * ir0[b]) * fma(1.0 / 24.0, br, (5.0 / 12.0) * k));
-        const double corr = u * fma(u, fma(u, q4, q3), -0.5 * e1);
+        const double corr = kepler_series_start(u, ir0[b], r0[b], eta[b], beta[b], mu);
         X[b] = abs_hi(corr) < 0x3fd00000 ? fma(u, corr, u) : u;  // |corr| < 0.25
     }
-    int ok[B];
-    // uniform = true_type: called with all lanes of amask converged; the choice of the Stumpff path is then one vote and a
-    // warp-uniform branch (the general path returns the series' values for small arguments, bit for bit)
-    auto iterate = [&](auto uniform) -> bool {
+    auto iterate = [&]() -> bool {
         double X2[B], z[B];
         Stumpff cs[B];
         int zmax = 0;
@@ -191,9 +192,7 @@ __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[
             z[b] = beta[b] * X2[b];
             zmax = max(zmax, abs_hi(z[b]));
         }
-        bool series = zmax < kHi0p1;
-        if constexpr (decltype(uniform)::value) series = __ballot_sync(amask, !series) == 0u;
-        if (__builtin_expect(series, 1)) {
+        if (zmax < kHi0p1) {
 #pragma unroll
             for (int b = 0; b < B; ++b) stumpff_series(z[b], cs[b].c0, cs[b].c1, cs[b].c2, cs[b].c3);
         } else {
@@ -215,28 +214,100 @@ __device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[
             X[b] -= dX;
             d[b] = -dX;
             // converged when the step is small relative to X AND as an angle (beta dX^2 = the square of the step in
-            // eccentric anomaly): the error left by a Chebyshev step is of the order of the cube of that angle, which
-            // for steps of many revolutions (X large) is not small just because dX / X is
+            // eccentric anomaly): the error left by a Chebyshev step is of the order of the cube of that angle,
+            // which for steps of many revolutions (X large) is not small just because dX / X is
             ok[b] = (abs_hi(dX) <= abs_hi(kConv * X[b])) & (abs_hi((beta[b] * dX) * dX) <= kHiConv2) &
                     (abs_hi(X[b]) < kHiInf);
             conv &= ok[b];
         }
         return conv != 0;
     };
-    // With the series start one evaluation is the rule (the step it yields is below kConv |X|, which confirms
-    // convergence): straight-line code for it, a loop only for the later ones (long steps, high eccentricity).
-    bool done = iterate(std::true_type{});
-    if (__builtin_expect(__ballot_sync(amask, !done) != 0u, 0)) {  // warp-uniform: some lane needs more
-        for (int it = 1; it < 50 && !done; ++it) done = iterate(std::false_type{});
-        if (!done) {  // some planet of this lane did not converge within the cap (or went non-finite): bisect those
+    bool done = iterate();
+    for (int it = 1; it < 50 && !done; ++it) done = iterate();
+    if (!done) {  // some planet of this lane did not converge within the cap (or went non-finite): bisect those
 #pragma unroll
-            for (int b = 0; b < B; ++b) {
-                if (!ok[b]) {
-                    X[b] = kepler_bisect(r0[b], eta[b], mu, beta[b], tau);
-                    g[b] = kepler_G(beta[b], X[b]);
-                    d[b] = 0.0;
-                }
+        for (int b = 0; b < B; ++b) {
+            if (!ok[b]) {
+                X[b] = kepler_bisect(r0[b], eta[b], mu, beta[b], tau);
+                g[b] = kepler_G(beta[b], X[b]);
+                d[b] = 0.0;
             }
+        }
+    }
+}
+
+template <int B, class Valid>
+__device__ __forceinline__ void kepler_drift_all(double (&Q)[B][3], double (&P)[B][3], double mu, double tau,
+                                                 unsigned amask, Valid valid) {
+    double r0[B], ir0[B], eta[B], beta[B], X[B], d[B];
+    KeplerG g[B];
+    // The common case -- a step of a few per cent of a period -- is straight-line code with every test folded into one
+    // flag (high words, integer ALU) and one vote: series start, ONE Stumpff series evaluation, one Chebyshev step.  It
+    // stands when, for every planet of the lane, the start's correction is below 0.25, the Stumpff argument and the
+    // Chebyshev correction are below 0.1, and the step taken is below 2^-18 |X| (with |z| < 0.1 that also bounds the
+    // step as an angle: beta dX^2 < 0.1 * 2^-36).  Otherwise the lane redoes its planets with the general procedure
+    // (kepler_general_solve: the same start and first iteration with their branches, then as many more as needed).
+    // Where the fast path stands it has computed exactly what the general procedure computes: same results, bit for bit.
+    int hcorr = 0, hz = 0, hc = 0, hX = 0, t1 = -0x7fffffff;
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+        const double r02 = fma(Q[b][2], Q[b][2], fma(Q[b][1], Q[b][1], Q[b][0] * Q[b][0]));
+        eta[b] = fma(Q[b][2], P[b][2], fma(Q[b][1], P[b][1], Q[b][0] * P[b][0]));
+        const double v2 = fma(P[b][2], P[b][2], fma(P[b][1], P[b][1], P[b][0] * P[b][0]));
+        ir0[b] = rsqrt_f64(r02);
+        r0[b] = r02 * ir0[b];
+        beta[b] = fma(2.0 * mu, ir0[b], -v2);
+        // Starting value: the universal Kepler equation is the power series
+        //   tau = r0 X + eta X^2 / 2 + (mu - beta r0) X^3 / 6 - beta eta X^4 / 24 + ...
+        // and its reversion to fourth order in u = tau / r0,
+        //   X = u (1 + u (q2 + u (q3 + u q4))),   q2 = -e1 / 2,  q3 = e1^2 / 2 - k / (6 r0),
+        //   q4 = e1 (5 k / 12 + beta r0 / 24) / r0 - 5 e1^3 / 8,   e1 = eta / r0,  k = mu - beta r0,
+        // is within 1e-6 of the root for steps of a few per cent of a period (config 4: max 7e-7), so that ONE
+        // Chebyshev step reaches rounding level; the plain guess X = u (the oracle's, R-M4) needs two.  Same root.
+        // Steps too long for the series (correction not small) start from X = u (kepler_general_solve).
+        const double u = tau * ir0[b];
+        const double corr = kepler_series_start(u, ir0[b], r0[b], eta[b], beta[b], mu);
+        X[b] = fma(u, corr, u);
+        hcorr = max(hcorr, abs_hi(corr));
+    }
+    {
+        double X2[B], z[B];
+        Stumpff cs[B];
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            X2[b] = X[b] * X[b];
+            z[b] = beta[b] * X2[b];
+            hz = max(hz, abs_hi(z[b]));
+            stumpff_series(z[b], cs[b].c0, cs[b].c1, cs[b].c2, cs[b].c3);
+        }
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+            g[b] = kepler_G_from(cs[b], X[b], X2[b]);
+            const double F = fma(r0[b], g[b].G1, fma(eta[b], g[b].G2, fma(mu, g[b].G3, -tau)));
+            const double r = fma(r0[b], g[b].G0, fma(eta[b], g[b].G1, mu * g[b].G2));
+            const double F2 = fma(eta[b], g[b].G0, fma(-beta[b], r0[b], mu) * g[b].G1);
+            const double ir = rcp_f64<false>(r);
+            const double d1 = F * ir;
+            const double c = (0.5 * d1) * (F2 * ir);
+            hc = max(hc, abs_hi(c));
+            const double dX = fma(d1, c, d1);
+            X[b] -= dX;
+            d[b] = -dX;
+            const int hx = abs_hi(X[b]);
+            t1 = max(t1, abs_hi(dX) - hx);  // |dX| <= 2^-18 |X|  <=>  high words differ by at least 18 << 20
+            hX = max(hX, hx);
+        }
+    }
+    const bool redo = (hcorr >= 0x3fd00000) | (hz >= kHi0p1) | (hc >= kHi0p1) | (t1 > -0x01200000) | (hX >= kHiInf);
+
+    if (__builtin_expect(__ballot_sync(amask, redo) != 0u, 0)) {  // warp-uniform, rarely taken
+        if (redo) {
+            KeplerLane<B> s;
+#pragma unroll
+            for (int b = 0; b < B; ++b) s.r0[b] = r0[b], s.ir0[b] = ir0[b], s.eta[b] = eta[b], s.beta[b] = beta[b];
+            kepler_general_solve<B>(s, mu, tau);
+#pragma unroll
+            for (int b = 0; b < B; ++b) X[b] = s.X[b], d[b] = s.d[b], g[b] = s.g[b];
         }
     }
 #pragma unroll
