@@ -29,6 +29,18 @@ __device__ __forceinline__ double pair_acc(const double (&xi)[3], double mi, dou
     return r2;
 }
 
+// the tracked minimum's high word, and the exact minimum (recomputed from the positions when only the high word was kept)
+__device__ __forceinline__ unsigned r2_high_word(u64 v) { return (unsigned)(v >> 32); }
+__device__ __forceinline__ unsigned r2_high_word(unsigned v) { return v; }
+template <int N, int L, int B>
+__device__ __forceinline__ u64 r2_exact(u64 tracked, const double (&)[B][3], int, int, unsigned) {
+    return tracked;
+}
+template <int N, int L, int B>
+__device__ __forceinline__ u64 r2_exact(unsigned, const double (&x)[B][3], int l, int base, unsigned mask) {
+    return pair_r2min<N, L, B>(x, l, base, mask);
+}
+
 // Shared memory of the cross-lane schedule (L > 1 only), per warp, in 16-byte words, word-major (word w of lane n at
 // [w * 32 + n]):  B * 2 words per lane: (x0, x1) (x2, m) of each of the lane's bodies.
 template <int L, int B>
@@ -42,13 +54,21 @@ __host__ __device__ constexpr int acc_ring_smem_words() {
 // shared memory (W = this warp's acc_ring_smem_words) and reads the visiting body right before the B pairs that use it;
 // the visitor's halves go back by shuffle and are added one visit behind, so that no instruction waits on a shuffle
 // that was just issued.
-template <int P, int L, int B>
+template <int P, int L, int B, class R2>
 __device__ __forceinline__ void eval_acc_planets(const double (&Q)[B][3], const double (&m)[B], double (&A)[B][3],
-                                                 u64& r2min, int l, int base, unsigned amask, double2* W) {
+                                                 R2& r2min, int l, int base, unsigned amask, double2* W) {
     constexpr bool PADDED = (L * B != P);
 #pragma unroll
     for (int b = 0; b < B; ++b) A[b][0] = A[b][1] = A[b][2] = 0.0;
-    r2min = ~0ull;
+    // r2min: the smallest squared separation this lane saw, tracked on the integer ALU either as the HIGH WORD of its bit
+    // pattern (R2 = unsigned: one integer min per pair; pair_r2min gives the exact value when the stop logic needs it) or
+    // as the full pattern (R2 = u64: a 64-bit compare and select per pair).  The caller chooses: the high word is faster
+    // for the one-system-per-thread shapes, the many-lane Cash-Karp shapes are faster with the full pattern (measured).
+    r2min = (R2)~(R2)0;
+    auto track = [&](double r2, bool valid) {
+        if constexpr (sizeof(R2) == 8) min_bits(r2min, r2, valid);
+        else min_hi(r2min, r2, valid);
+    };
     if constexpr (L > 1) {
         const int wl = threadIdx.x & 31;
         __syncwarp(amask);  // every lane has finished reading the previous publication
@@ -64,7 +84,7 @@ __device__ __forceinline__ void eval_acc_planets(const double (&Q)[B][3], const 
 #pragma unroll
         for (int c = b + 1; c < B; ++c) {
             const double r2 = pair_acc(Q[b], m[b], A[b], Q[c], m[c], A[c]);
-            min_bits(r2min, r2, !PADDED || (l * B + c < P));
+            track(r2, !PADDED || (l * B + c < P));
         }
     if constexpr (L > 1) {
         constexpr int H = (L - 1) / 2;
@@ -87,7 +107,7 @@ __device__ __forceinline__ void eval_acc_planets(const double (&Q)[B][3], const 
 #pragma unroll
                 for (int b = 0; b < B; ++b) {
                     const double r2 = b == 0 ? pair_acc<true>(Q[b], m[b], A[b], xv, mv, av) : pair_acc(Q[b], m[b], A[b], xv, mv, av);
-                    min_bits(r2min, r2, vvalid && (!PADDED || (l * B + b < P)));
+                    track(r2, vvalid && (!PADDED || (l * B + b < P)));
                 }
                 if (vis >= 1) {  // sent one visit ago
 #pragma unroll

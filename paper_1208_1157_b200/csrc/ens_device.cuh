@@ -53,4 +53,41 @@ __device__ __forceinline__ void min_hi(unsigned& acc, double r2, bool valid = tr
     acc = min(acc, h);
 }
 
+
+// Smallest squared pair separation of the N bodies a group of L lanes holds (bit pattern), positions only, in the
+// arithmetic of the pair evaluations (dx = x_k - x_i; r^2 = fma(dz, dz, fma(dy, dy, dx dx))): the exact value behind
+// the high words the step loops track.  Used by the exact stop logic of every kernel and by the close-approach monitor
+// of the 2-evaluation Hermite variant.  Same lane ring as the evaluations, by shuffle; no return traffic (each lane
+// keeps the minimum over the pairs it sees; the caller reduces the flag over the lanes).
+template <int N, int L, int B>
+__device__ __forceinline__ u64 pair_r2min(const double (&x)[B][3], int l, int base, unsigned amask) {
+    constexpr bool PADDED = (L * B != N);
+    u64 r2min = ~0ull;
+    auto d2 = [](const double (&p)[3], const double (&q)[3]) {
+        const double dx = q[0] - p[0], dy = q[1] - p[1], dz = q[2] - p[2];
+        return fma(dz, dz, fma(dy, dy, dx * dx));
+    };
+#pragma unroll
+    for (int b = 0; b < B; ++b)
+#pragma unroll
+        for (int c = b + 1; c < B; ++c) min_bits(r2min, d2(x[b], x[c]), !PADDED || (l * B + c < N));
+    if constexpr (L > 1) {
+#pragma unroll
+        for (int s = 1; s <= (L - 1) / 2; ++s) {
+            int ls = l + s;
+            if (ls >= L) ls -= L;
+#pragma unroll
+            for (int c = 0; c < B; ++c) {
+                double xv[3];
+#pragma unroll
+                for (int q = 0; q < 3; ++q) xv[q] = __shfl_sync(amask, x[c][q], base + ls);
+                const bool vvalid = !PADDED || (ls * B + c < N);
+#pragma unroll
+                for (int b = 0; b < B; ++b) min_bits(r2min, d2(x[b], xv), vvalid && (!PADDED || (l * B + b < N)));
+            }
+        }
+    }
+    return r2min;
+}
+
 }  // namespace ensd

@@ -448,7 +448,7 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
     const bool mon_close = p.rc2_bits != 0ull;
     const bool mon_eject = p.re2_bits < 0x7FEFFFFFFFFFFFFFull;
     int64_t k = 0;
-    u64 r2min = ~0ull;
+    unsigned r2min = ~0u;  // high word of the smallest planet-pair r^2 of the last acceleration evaluation
     double s[3] = {0.0, 0.0, 0.0};
 
     // Alg. 1 loop test before the first step (R10): time first, then the step budget
@@ -565,11 +565,11 @@ __global__ void __maxnreg__(MAXREG) mvs_kernel(View e, StepArgs p) {
             }
             const unsigned xhi = max(max((unsigned)__double2hiint(Xm[0]) & 0x7fffffffu, (unsigned)__double2hiint(Xm[1]) & 0x7fffffffu),
                                      (unsigned)__double2hiint(Xm[2]) & 0x7fffffffu);
-            const bool go = ((unsigned)(r2min >> 32) > (unsigned)(p.rc2_bits >> 32)) && (qlo > p.rc1_hi) && (qhi < p.ceq_hi) &&
+            const bool go = (r2min > (unsigned)(p.rc2_bits >> 32)) && (qlo > p.rc1_hi) && (qhi < p.ceq_hi) &&
                             (xhi < p.cex_hi) && (ts < p.te) && (k < p.max_steps);
             if (__builtin_expect(__ballot_sync(am, !go) != 0u, 0)) {
                 int f = 0;
-                if (mon_close && r2min < p.rc2_bits) f |= 1;
+                if (mon_close && pair_r2min<P, L, B>(Qm, l, base, am) < p.rc2_bits) f |= 1;
                 u64 q2max = 0ull, q2min = ~0ull;  // over this lane's planets: star-planet separation is |Q_i|
 #pragma unroll
                 for (int b = 0; b < B; ++b) {

@@ -16,6 +16,7 @@
 // and MVS kernels (L lanes per system, B bodies per lane; the pair evaluation is acc_pairs.cuh's acceleration-only ring
 // over all N bodies).
 #pragma once
+#include <type_traits>
 #include "acc_pairs.cuh"
 
 namespace ensd {
@@ -76,7 +77,9 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
     const double h = p.dt;
     int64_t k = 0;
     double K[5][B][3];  // stage accelerations k_1 .. k_5
-    u64 r2min;
+    // smallest pair r^2 of stage 1: its high word (one system per thread) or its full bit pattern (acc_pairs.cuh)
+    using R2 = typename std::conditional<(L > 1), u64, unsigned>::type;
+    R2 r2min;
 
     // The systems of the warp that run enter the loop together (mask amask) and stay in it until the exact stop logic
     // retires them (hermite_kernel.cuh): one vote and one almost never taken branch per step.
@@ -95,10 +98,10 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c)
                     if (!PADDED || (l * B + b < N)) cmax = max(cmax, (unsigned)__double2hiint(X[b][c]) & 0x7fffffffu);
-            const bool go = ((unsigned)(r2min >> 32) > (unsigned)(p.rc2_bits >> 32)) && (cmax < p.ce_hi) && (ts < p.te) &&
+            const bool go = (r2_high_word(r2min) > (unsigned)(p.rc2_bits >> 32)) && (cmax < p.ce_hi) && (ts < p.te) &&
                             (k < p.max_steps);
             if (__builtin_expect(__ballot_sync(amask, !go) != 0u, 0)) {
-                int f = (r2min < p.rc2_bits) ? 1 : 0;
+                int f = (r2_exact<N, L, B>(r2min, X, l, base, amask) < p.rc2_bits) ? 1 : 0;
 #pragma unroll
                 for (int b = 0; b < B; ++b) {
                     const u64 db = dbits(fma(X[b][2], X[b][2], fma(X[b][1], X[b][1], X[b][0] * X[b][0])));
@@ -136,7 +139,7 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
             {
                 const unsigned am2 = amask;
                 double Xs[B][3], K6[B][3];
-                u64 dummy;
+                R2 dummy;
 #pragma unroll
                 for (int i = 1; i < 6; ++i) {  // stages 2 .. 6
 #pragma unroll
@@ -328,7 +331,9 @@ __global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkU
     };
 
     double K[5][B][3];  // stage accelerations k_1 .. k_5
-    u64 r2min;
+    // smallest pair r^2 of stage 1: its high word (one system per thread) or its full bit pattern (acc_pairs.cuh)
+    using R2 = typename std::conditional<(L > 1), u64, unsigned>::type;
+    R2 r2min;
 
     while (true) {
         if (!refill()) break;
@@ -348,10 +353,10 @@ __global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkU
 #pragma unroll
                     for (int c = 0; c < 3; ++c)
                         if (!PADDED || (l * B + b < N)) cmax = max(cmax, (unsigned)__double2hiint(X[b][c]) & 0x7fffffffu);
-                const bool go = ((unsigned)(r2min >> 32) > (unsigned)(p.rc2_bits >> 32)) && (cmax < p.ce_hi) &&
+                const bool go = (r2_high_word(r2min) > (unsigned)(p.rc2_bits >> 32)) && (cmax < p.ce_hi) &&
                                 (fwd ? (t < p.t_end) : (t > p.t_end)) && (k < p.max_steps);
                 if (__builtin_expect(__ballot_sync(kmask, !go) != 0u, 0)) {
-                    int f = (r2min < p.rc2_bits) ? 1 : 0;
+                    int f = (r2_exact<N, L, B>(r2min, X, l, base, kmask) < p.rc2_bits) ? 1 : 0;
 #pragma unroll
                     for (int b = 0; b < B; ++b) {
                         const u64 db = dbits(fma(X[b][2], X[b][2], fma(X[b][1], X[b][1], X[b][0] * X[b][0])));
@@ -387,7 +392,7 @@ __global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkU
             if (active) {
                 const double h2 = h * h;
                 double Xs[B][3], K6[B][3];
-                u64 dummy;
+                R2 dummy;
 #pragma unroll
                 for (int i = 1; i < 6; ++i) {  // stages 2 .. 6
                     const double ch = q.c[i] * h;
