@@ -91,12 +91,12 @@ def rkck_adaptive_work(n_body: int):
 
 
 def mvs_work(n_body: int, merged: bool = False):
-    """Per planet: universal-variable Kepler drift 113 (setup 16, series start 19, one 7-term Stumpff evaluation +
-    Chebyshev step 41, Taylor finish + f, g functions 37), drifts / kicks / momentum sum 15 (merged: 12); per system 16
+    """Per planet: universal-variable Kepler drift 111 (setup 17, series start 18, one 7-term Stumpff evaluation +
+    Chebyshev step 39 with its tests on the integer ALU, Taylor finish + f, g functions 37), drifts / kicks / momentum sum 15 (merged: 12); per system 16
     (merged: 13); planet pairs 21 each.  The monitors cost no FP64 instruction (high words, integer ALU)."""
     pl = n_body - 1
     pp = _pairs(pl)
-    per_planet_i, per_planet_f = (113 + 12, 173 + 20) if merged else (113 + 15, 173 + 24)
+    per_planet_i, per_planet_f = (111 + 12, 172 + 20) if merged else (111 + 15, 172 + 24)
     per_sys_i, per_sys_f = (13, 19) if merged else (16, 22)
     return pl * per_planet_i + per_sys_i + pp * ACC_PAIR_INSTR, pl * per_planet_f + per_sys_f + pp * ACC_PAIR_FLOPS
 

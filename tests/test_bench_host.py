@@ -24,7 +24,7 @@ def test_work_models_of_the_other_kernels():
     # the counts quoted there for the tuned shapes
     assert bench.hermite_carry_work(3)[0] == 400 and bench.rkck_work(3)[0] == 604
     assert bench.hermite_adaptive_work(3)[0] == 496 + 62
-    assert bench.mvs_work(4)[0] == 3 * 128 + 16 + 3 * 21 == 463 and bench.mvs_work(4, merged=True)[0] == 451
+    assert bench.mvs_work(4)[0] == 3 * 126 + 16 + 3 * 21 == 457 and bench.mvs_work(4, merged=True)[0] == 445
     assert bench.rkck_adaptive_work(3)[0] > bench.rkck_work(3)[0]
     for kind, fn in bench.WORK.items():
         for n in range(2, 17):
