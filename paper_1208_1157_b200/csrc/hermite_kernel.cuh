@@ -8,16 +8,19 @@
 // Work split (differs from the paper's Fermi design): a system is held by L lanes of a warp (L odd),
 // B bodies per lane.  Every unordered pair is evaluated exactly once:
 //   * pairs of two bodies of the same lane: in registers;
-//   * pairs across lanes: ring schedule.  At shift s = 1..(L-1)/2 lane l fetches the bodies of lane (l+s) mod L
-//     with warp shuffles, accumulates its own half of each pair in registers and the visitor's half (Newton's
-//     third law) in a temporary that is shuffled back to the owner.  No shared memory, no __syncthreads.
-// L = 1 (n_body <= 8) is "one system per thread" and contains no shuffle at all.
+//   * pairs across lanes: ring schedule.  At shift s = 1..(L-1)/2 lane l is visited by the bodies of lane (l+s) mod L
+//     (read from the warp's own shared memory, where every lane publishes its bodies once per evaluation),
+//     accumulates its own half of each pair in registers and the visitor's half (Newton's third law) in a temporary
+//     that goes back to the owner by shuffle or through the owner's shared-memory slot.  No __syncthreads.
+// L = 1 (n_body <= 8) is "one system per thread" and touches neither shared memory nor shuffles.
 //
 // The first evaluation of step k+1 is the evaluation of the post-step-k state, so its minimum pair distance IS
 // the close-approach monitor Alg. 1 places after step k: monitors cost no extra pair work, and a
-// launch costs 3 evaluations per step + 1.  A system that stops (monitor, t_end, step budget) goes inactive;
-// the warp keeps looping only while some lane is active and inactive lanes skip the step body, so finished
-// systems consume no FP64 issue slots (north_star item 3).
+// launch costs 3 evaluations per step + 1.  The monitors and the loop tests are one quick test per step on high words
+// (integer ALU) and one vote; the exact logic runs behind a warp-uniform, rarely taken branch (quick_test, exact_stop).
+// A system that stops (monitor, t_end, step budget) leaves the step loop; the other systems of the warp go on under
+// the reduced mask and the warp is done when none is left, so finished systems consume no FP64 issue slots
+// (north_star item 3).
 #pragma once
 #include "ens_device.cuh"
 

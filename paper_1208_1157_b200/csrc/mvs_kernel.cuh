@@ -11,12 +11,14 @@
 //      V_i += h/2 A_i                                                      P:L256)
 //   5  Q_i += h/2 s (s from the new V; the SAME s opens the next step), X_cm += h/2 V_cm
 // The Kepler drift uses universal variables (BASELINE.json config 4; R-M3, R-M4): solve
-//   r0 G1 + eta G2 + mu G3 = tau,  G_n = X^n c_n(beta X^2),  by Newton from X = tau / r0, then the f and g functions.
+//   r0 G1 + eta G2 + mu G3 = tau,  G_n = X^n c_n(beta X^2),  then the f and g functions (kepler_drift_all: a straight-line
+// fast path for steps of a few per cent of a period, the general procedure out of line).
 //
 // Work split: L lanes per system (L odd), B planets per lane; the Kepler drift is per planet and needs no
-// communication; planet-planet pairs use the same in-lane + ring-of-shuffles schedule as the Hermite kernel; the
+// communication; planet-planet pairs use the same in-lane + lane-ring schedule as the Hermite kernel (acc_pairs.cuh); the
 // momentum sum of the Cartesian drift is an L-lane all-gather of per-lane partial sums.  L = 1 (n_body <= 9) is
-// one system per thread with the oracle's summation order and no shuffle.
+// one system per thread with the oracle's summation order and no shuffle.  Monitors and loop tests: one quick test per
+// step on high words and one vote, the exact logic behind a warp-uniform, rarely taken branch (as in hermite_kernel.cuh).
 #pragma once
 #include <cfloat>
 #include <type_traits>
