@@ -310,6 +310,9 @@ def main():
                     help="Hermite workload (BASELINE.json configs index); 1 is the metric's, the others are for profiling")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg (profiling runs)")
     ap.add_argument("--no-extras", action="store_true", help="skip the e2e / other-kernel / HBM legs (profiling runs)")
+    ap.add_argument("--n-sys", type=int, default=None,
+                    help="profiling runs: another ensemble size of the same workload (e.g. 18944 = one warp per SM "
+                         "sub-partition at n_body = 3); the line says so and is not the metric")
     ap.add_argument("--only", default=None,
                     help="profiling runs: launch just this entry of other_workloads (e.g. mvs_131072x4) a few times and exit")
     args = ap.parse_args()
@@ -345,6 +348,9 @@ def main():
     stream = torch.cuda.Stream()
     c = W.CONFIGS[CFG]
     n_sys, n_body = c.n_sys, c.n_body
+    if args.n_sys:
+        n_sys = int(args.n_sys)
+        print(f"bench.py: --n-sys {n_sys}: not the metric's ensemble ({c.n_sys}); the number is for profiling only", file=sys.stderr)
 
     # the other step-loop kernels (kernel time only; none of them the metric).  name -> arguments of time_kernel
     def others_table():
