@@ -10,14 +10,15 @@ namespace {
 // n_body -> lanes per system L (odd), bodies per lane B, L * B >= n_body.  Exact fits for 2-6, 9, 10, 12, 15;
 // the others run in the next larger shape with massless dummy slots.  The values are the winners of the sweeps
 // recorded in DESIGN.md section 8 (tuning record).
-//   UNROLL   three inlined copies of the evaluation (straight-line step) instead of a 3-phase loop around one copy
+//   UNROLL   1: three inlined copies of the evaluation (straight-line step); 2: two (the corrector iterations are a loop
+//            around one); 0: a 3-phase loop around one copy
 //   THREADS  threads per block;  MAXT, MINB = __launch_bounds__ (register cap 65536 / (MAXT * MINB))
 //   MODE     0 = fixed step (3 evaluations), 1 = adaptive step, 2 = carried a, j (2 evaluations), 3 = MODE 0 time-sliced
 template <int N> struct ShapeBase;
 #define ENS_SHAPE(N_, L_, B_, UNROLL_, THREADS_, MINB_, MAXT_)                              \
     template <> struct ShapeBase<N_> {                                                      \
         static constexpr int L = L_, B = B_, THREADS = THREADS_, MINB = MINB_, MAXT = MAXT_; \
-        static constexpr bool UNROLL = UNROLL_;                                             \
+        static constexpr int UNROLL = UNROLL_;                                              \
     };
 // the shape of (N, MODE): the per-N entry unless a mode has its own launch bounds below (L and B never differ by mode)
 template <int N, int MODE> struct ShapeOf : ShapeBase<N> {};
@@ -25,37 +26,40 @@ template <int N, int MODE> struct ShapeOf : ShapeBase<N> {};
     template <> struct ShapeOf<N_, MODE_> {                                                              \
         static constexpr int L = ShapeBase<N_>::L, B = ShapeBase<N_>::B, THREADS = THREADS_, MINB = MINB_, \
                              MAXT = MAXT_;                                                               \
-        static constexpr bool UNROLL = UNROLL_;                                                          \
+        static constexpr int UNROLL = UNROLL_;                                                           \
     };
 //        N  L  B  unroll threads minBlocks maxThreads
-ENS_SHAPE(2, 1, 2, true, 64, 1, 128)
+ENS_SHAPE(2, 1, 2, 1, 64, 1, 128)
 // n_body = 3 (config 1, the metric): register cap 128 (125 used, no spills), 8 blocks of 2 warps per SM
-ENS_SHAPE(3, 1, 3, true, 64, 7, 64)
-ENS_SHAPE(4, 1, 4, true, 64, 1, 128)
-ENS_SHAPE(5, 1, 5, true, 64, 1, 128)
+ENS_SHAPE(3, 1, 3, 1, 64, 7, 64)
+ENS_SHAPE(4, 1, 4, 1, 64, 1, 128)
+ENS_SHAPE(5, 1, 5, 1, 64, 1, 128)
 // n_body = 6 (config 2): one system per thread, all 15 pairs in one lane, no shuffles: 0.62 of FP64 issue peak against
 // 0.54 for the best 3-lane shape; 32-thread blocks spread the 1024 warps of config 2 evenly over the SMs; straight-line
-// step 0.668 against 0.653 for the 3-phase loop
-ENS_SHAPE(6, 1, 6, true, 32, 1, 32)
+// step 0.668 against 0.653 for the 3-phase loop; with the corrector iterations rolled (24 KB of code per step instead of
+// 35 KB) 0.730 against 0.689
+ENS_SHAPE(6, 1, 6, 2, 32, 1, 32)
 // n_body = 7, 8: still one system per thread.  The state no longer fits 255 registers (336 / 664 B of it live in
 // local memory, L1-resident: the step loop touches no other memory), yet every lane does useful work and nothing is
 // shuffled: 0.65 / 0.63 of FP64 issue peak against 0.36 / 0.46 for 3 lanes x 3 bodies (9 slots for 7 or 8 bodies).
-// From n_body = 9 on the spill traffic wins (0.44 against 0.59) and the lane-split shapes take over.
-ENS_SHAPE(7, 1, 7, false, 32, 1, 32)
-ENS_SHAPE(8, 1, 8, false, 32, 1, 32)
-ENS_SHAPE(9, 3, 3, false, 64, 1, 128)
+// From n_body = 9 on the spill traffic wins (0.44 against 0.59) and the lane-split shapes take over.  Two copies of
+// the evaluation (rolled corrector iterations) spill less than the 3-phase loop around one (112 / 552 B against
+// 336 / 688 B) and are 3 - 4 % faster.
+ENS_SHAPE(7, 1, 7, 2, 32, 1, 32)
+ENS_SHAPE(8, 1, 8, 2, 32, 1, 32)
+ENS_SHAPE(9, 3, 3, 0, 64, 1, 128)
 // n_body = 10 (the paper's largest Table 3 shape): 168 registers -> 12 warps per SM: 0.60 against 0.54 at 242 registers
-ENS_SHAPE(10, 5, 2, false, 64, 3, 128)
-ENS_SHAPE(11, 3, 4, false, 64, 1, 128)
-ENS_SHAPE(12, 3, 4, false, 64, 1, 128)
-ENS_SHAPE(13, 5, 3, false, 64, 1, 128)
-ENS_SHAPE(14, 5, 3, false, 64, 1, 128)
-ENS_SHAPE(15, 5, 3, false, 64, 1, 128)
-ENS_SHAPE(16, 5, 4, false, 64, 1, 128)
+ENS_SHAPE(10, 5, 2, 0, 64, 3, 128)
+ENS_SHAPE(11, 3, 4, 0, 64, 1, 128)
+ENS_SHAPE(12, 3, 4, 0, 64, 1, 128)
+ENS_SHAPE(13, 5, 3, 0, 64, 1, 128)
+ENS_SHAPE(14, 5, 3, 0, 64, 1, 128)
+ENS_SHAPE(15, 5, 3, 0, 64, 1, 128)
+ENS_SHAPE(16, 5, 4, 0, 64, 1, 128)
 // the carried accelerations and jerks are 18 more live doubles at n_body = 3: 128 registers spilled 120 B of them
-ENS_SHAPE_MODE(3, 2, true, 64, 5, 64)
+ENS_SHAPE_MODE(3, 2, 1, 64, 5, 64)
 // n_body = 6 with carried a, j: the straight-line step spilled 464 B; the 3-phase loop spills 16 B and is 3.7 % faster
-ENS_SHAPE_MODE(6, 2, false, 32, 1, 32)
+ENS_SHAPE_MODE(6, 2, 0, 32, 1, 32)
 #undef ENS_SHAPE
 #undef ENS_SHAPE_MODE
 

@@ -273,9 +273,10 @@ __device__ __forceinline__ int monitor_flags(const double (&x)[B][3], unsigned r
     return f & 7;
 }
 
-// UNROLL = true: the three evaluations of a step are three inlined copies (straight-line step, best for small
-// pair counts); false: one copy of the evaluation inside a 3-phase loop (keeps large-n kernels inside the
-// instruction cache and the live register set at x, v, C_x, C_v, a, j).
+// UNROLL = 1: the three evaluations of a step are three inlined copies (straight-line step, best for small pair
+// counts); 2: the same with the two corrector iterations as one copy in a loop (two copies of the evaluation);
+// 0: one copy of the evaluation inside a 3-phase loop (keeps large-n kernels inside the instruction cache and the
+// live register set at x, v, C_x, C_v, a, j).
 // ADAPT = true: the adaptive-step integrator (Eq. 5): p.dt is the step size scale tau, the step h and the ten
 // coefficients are per system and per step (registers) instead of launch constants.
 // CARRY = true: Alg. 2 exactly as printed (reading R6-alt): two evaluations per step; (a0, j0) of a step
@@ -287,7 +288,7 @@ __device__ __forceinline__ int monitor_flags(const double (&x)[B][3], unsigned r
 // slice s) from a device counter, slice-major, so all groups advance at the same rate and an ensemble of, say, 1.15
 // waves of resident warps keeps every warp slot busy until the last slice instead of running a second, nearly empty
 // wave for a whole pass (config 3: DESIGN.md section 6.1).  slice_done[g] orders slice s + 1 of a group after slice s.
-template <int N, int L, int B, bool UNROLL, int MAXT, int MINB, bool ADAPT = false, bool CARRY = false,
+template <int N, int L, int B, int UNROLL, int MAXT, int MINB, bool ADAPT = false, bool CARRY = false,
           bool SLICED = false>
 __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p) {
     static_assert(!(ADAPT && CARRY), "the carried (a, j) are not kept across refills");
@@ -502,6 +503,23 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
             }
     };
 
+    // the two corrector iterations of the straight-line kernels: two inlined copies (UNROLL = 1) or one copy in a loop
+    // (UNROLL = 2: a third less code to fetch per step; faster where the straight-line step outgrows the instruction
+    // cache, n_body = 6: 35 KB)
+    auto corrector_iterations = [&](unsigned am) {
+        if constexpr (UNROLL == 2) {
+#pragma unroll 1
+            for (int it = 0; it < 2; ++it) {
+                eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am, W);
+                correct();
+            }
+        } else {
+            eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am, W);
+            correct();
+            eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am, W);
+            correct();
+        }
+    };
     bool fresh = true;  // CARRY: a, j do not yet belong to the current state (warp-uniform: start of the launch)
     auto run = [&]() {
     if constexpr (UNROLL && !ADAPT) {
@@ -523,10 +541,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                     if (!active) break;
                 }
                 predict(am);
-                eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am, W);
-                correct();
-                eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, am, W);
-                correct();
+                corrector_iterations(am);
             }
         }
     } else if constexpr (UNROLL) {
@@ -546,10 +561,7 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                         if (__ballot_sync(amask, active) != amask) break;  // some group retired its system
                     }
                     predict(amask);
-                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, amask, W);
-                    correct();
-                    eval_acc_jerk<N, L, B, false>(X, V, m, a, j, r2min, l, base, amask, W);
-                    correct();
+                    corrector_iterations(amask);
                 }
             }
         }
