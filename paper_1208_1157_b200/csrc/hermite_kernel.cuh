@@ -529,12 +529,12 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
         const unsigned amask0 = __ballot_sync(0xffffffffu, active);
         if (active) {
             unsigned am = amask0;
-            while (true) {
-                if (!CARRY || fresh)
-                    eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, am, W);
-                else
-                    r2min = p.rc2_bits ? (unsigned)(pair_r2min<N, L, B>(X, l, base, am) >> 32) : ~0u;
+            if constexpr (CARRY) {  // the one evaluation at the state itself (start of the launch), outside the loop
+                eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, am, W);
                 fresh = false;
+            }
+            while (true) {
+                if constexpr (!CARRY) eval_acc_jerk<N, L, B>(X, V, m, a, j, r2min, l, base, am, W);
                 if (__builtin_expect(quick_test(am) != 0u, 0)) {
                     exact_stop(am);
                     am = __ballot_sync(am, active);  // the lanes that go on
@@ -542,6 +542,9 @@ __global__ void __launch_bounds__(MAXT, MINB) hermite_kernel(View e, StepArgs p)
                 }
                 predict(am);
                 corrector_iterations(am);
+                // CARRY: (a, j) of the last corrector evaluation open the next step; its monitor needs the separations
+                // of the post-step state
+                if constexpr (CARRY) r2min = p.rc2_bits ? (unsigned)(pair_r2min<N, L, B>(X, l, base, am) >> 32) : ~0u;
             }
         }
     } else if constexpr (UNROLL) {
