@@ -12,6 +12,7 @@ template <int N> struct RkShape;
 #define ENS_RK_SHAPE_A(N_, L_, B_, THREADS_, MAXREG_, MAXREG_A_)                                         \
     template <> struct RkShape<N_> {                                                                     \
         static constexpr int L = L_, B = B_, THREADS = THREADS_, MAXREG = MAXREG_, MAXREG_A = MAXREG_A_; \
+        static constexpr bool ROLLED = (N_ == 7) || (L_ == 5 && B_ >= 3); /* fixed step: stages 2 .. 6 as a loop */ \
     };
 #define ENS_RK_SHAPE(N_, L_, B_, THREADS_, MAXREG_) ENS_RK_SHAPE_A(N_, L_, B_, THREADS_, MAXREG_, MAXREG_)
 //           N   L  B  threads maxRegisters
@@ -42,7 +43,7 @@ constexpr auto kernel_ptr() {
     if constexpr (ADAPT)
         return &rkck_adaptive_kernel<N, S::L, S::B, S::MAXREG_A>;
     else
-        return &rkck_kernel<N, S::L, S::B, S::MAXREG>;
+        return &rkck_kernel<N, S::L, S::B, S::MAXREG, S::ROLLED>;
 }
 
 template <int N, bool ADAPT = false>

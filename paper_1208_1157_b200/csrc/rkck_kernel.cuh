@@ -28,7 +28,12 @@ struct RkCoef {
     double hb[6];       // h b_i (fifth-order weights)
 };
 
-template <int N, int L, int B, int MAXREG>
+// ROLLED = true: stages 2 .. 6 are a loop around ONE copy of the evaluation, the stage accelerations live in local memory
+// (L1-resident; they are read back once per later stage) and only the current one is in registers.  For shapes whose
+// stage accelerations do not fit the registers anyway and whose straight-line step (six copies of the evaluation) no
+// longer fits the instruction cache: n_body = 7, one system per thread (48 KB of code, 1.3 instruction-fetch stalls
+// per issued instruction).  Same arithmetic in the same order.
+template <int N, int L, int B, int MAXREG, bool ROLLED = false>
 __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
     constexpr int S = 32 / L;
     constexpr bool PADDED = (L * B != N);
@@ -136,7 +141,50 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
                 amask = __ballot_sync(amask, active);  // the lanes that go on
                 if (!active) break;
             }
-            {
+            if constexpr (ROLLED) {
+                const unsigned am2 = amask;
+                double Xs[B][3], Kt[B][3];
+                double KL[6][B][3];  // k_1 .. k_6, indexed by the stage counter: local memory
+                R2 dummy;
+#pragma unroll
+                for (int b = 0; b < B; ++b)
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) KL[0][b][c] = K[0][b][c];
+#pragma unroll 1
+                for (int i = 1; i < 6; ++i) {  // stages 2 .. 6
+                    const double chi = q.ch[i];
+#pragma unroll
+                    for (int b = 0; b < B; ++b)
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) Xs[b][c] = fma(chi, V[b][c], X[b][c]);
+#pragma unroll 1
+                    for (int ll = 0; ll + 2 <= i; ++ll) {
+                        const double cf = q.h2AA[i][ll];
+#pragma unroll
+                        for (int b = 0; b < B; ++b)
+#pragma unroll
+                            for (int c = 0; c < 3; ++c) Xs[b][c] = fma(cf, KL[ll][b][c], Xs[b][c]);
+                    }
+                    eval_acc_planets<N, L, B>(Xs, m, Kt, dummy, l, base, am2, W);
+#pragma unroll
+                    for (int b = 0; b < B; ++b)
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) KL[i][b][c] = Kt[b][c];
+                }
+#pragma unroll
+                for (int b = 0; b < B; ++b)
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        double s = fma(h, V[b][c], X[b][c]);
+#pragma unroll
+                        for (int ll = 0; ll < 5; ++ll) s = fma(q.h2bA[ll], KL[ll][b][c], s);
+                        X[b][c] = s;
+                        double w = fma(q.hb[0], KL[0][b][c], V[b][c]);  // b_2 = b_5 = 0
+                        w = fma(q.hb[2], KL[2][b][c], w);
+                        w = fma(q.hb[3], KL[3][b][c], w);
+                        V[b][c] = fma(q.hb[5], Kt[b][c], w);
+                    }
+            } else {
                 const unsigned am2 = amask;
                 double Xs[B][3], K6[B][3];
                 R2 dummy;
@@ -169,9 +217,9 @@ __global__ void __maxnreg__(MAXREG) rkck_kernel(View e, StepArgs p, RkCoef q) {
                         w = fma(q.hb[3], K[3][b][c], w);
                         V[b][c] = fma(q.hb[5], K6[b][c], w);
                     }
-                ts += fabs(h);
-                ++k;
             }
+            ts += fabs(h);
+            ++k;
         }
     }
 
