@@ -12,7 +12,7 @@ template <int N> struct RkShape;
 #define ENS_RK_SHAPE_A(N_, L_, B_, THREADS_, MAXREG_, MAXREG_A_)                                         \
     template <> struct RkShape<N_> {                                                                     \
         static constexpr int L = L_, B = B_, THREADS = THREADS_, MAXREG = MAXREG_, MAXREG_A = MAXREG_A_; \
-        static constexpr bool ROLLED = (N_ == 7) || (L_ == 5 && B_ >= 3); /* fixed step: stages 2 .. 6 as a loop */ \
+        static constexpr bool ROLLED = (N_ == 7) || (L_ == 5 && B_ >= 3); /* stages 2 .. 6 as a loop (rkck_kernel.cuh) */ \
     };
 #define ENS_RK_SHAPE(N_, L_, B_, THREADS_, MAXREG_) ENS_RK_SHAPE_A(N_, L_, B_, THREADS_, MAXREG_, MAXREG_)
 //           N   L  B  threads maxRegisters
@@ -41,7 +41,7 @@ template <int N, bool ADAPT = false>
 constexpr auto kernel_ptr() {
     using S = RkShape<N>;
     if constexpr (ADAPT)
-        return &rkck_adaptive_kernel<N, S::L, S::B, S::MAXREG_A>;
+        return &rkck_adaptive_kernel<N, S::L, S::B, S::MAXREG_A, S::ROLLED>;
     else
         return &rkck_kernel<N, S::L, S::B, S::MAXREG, S::ROLLED>;
 }

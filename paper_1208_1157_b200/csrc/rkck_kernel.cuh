@@ -277,7 +277,7 @@ __device__ __forceinline__ double inv_fifth_root(double r) {
     return y;
 }
 
-template <int N, int L, int B, int MAXREG>
+template <int N, int L, int B, int MAXREG, bool ROLLED = false>
 __global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkUnit q) {
     constexpr int S = 32 / L;
     constexpr bool PADDED = (L * B != N);
@@ -440,24 +440,63 @@ __global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkU
             if (active) {
                 const double h2 = h * h;
                 double Xs[B][3], K6[B][3];
+                double KL[ROLLED ? 6 : 1][B][3];  // ROLLED (see rkck_kernel): k_1 .. k_6 in local memory, one copy of the evaluation
                 R2 dummy;
-#pragma unroll
-                for (int i = 1; i < 6; ++i) {  // stages 2 .. 6
-                    const double ch = q.c[i] * h;
+                if constexpr (ROLLED) {
 #pragma unroll
                     for (int b = 0; b < B; ++b)
 #pragma unroll
-                        for (int c = 0; c < 3; ++c) {
-                            double s = 0.0;
+                        for (int c = 0; c < 3; ++c) KL[0][b][c] = K[0][b][c];
+#pragma unroll 1
+                    for (int i = 1; i < 6; ++i) {  // stages 2 .. 6
+                        const double ch = q.c[i] * h;
+                        double S[B][3];
 #pragma unroll
-                            for (int ll = 0; ll + 2 <= i; ++ll) s = fma(q.AA[i][ll], K[ll][b][c], s);
-                            Xs[b][c] = fma(h2, s, fma(ch, V[b][c], X[b][c]));
+                        for (int b = 0; b < B; ++b)
+#pragma unroll
+                            for (int c = 0; c < 3; ++c) S[b][c] = 0.0;
+#pragma unroll 1
+                        for (int ll = 0; ll + 2 <= i; ++ll) {
+                            const double cf = q.AA[i][ll];
+#pragma unroll
+                            for (int b = 0; b < B; ++b)
+#pragma unroll
+                                for (int c = 0; c < 3; ++c) S[b][c] = fma(cf, KL[ll][b][c], S[b][c]);
                         }
-                    if (i < 5)
-                        eval_acc_planets<N, L, B>(Xs, m, K[i], dummy, l, base, am2, W);
-                    else
+#pragma unroll
+                        for (int b = 0; b < B; ++b)
+#pragma unroll
+                            for (int c = 0; c < 3; ++c) Xs[b][c] = fma(h2, S[b][c], fma(ch, V[b][c], X[b][c]));
                         eval_acc_planets<N, L, B>(Xs, m, K6, dummy, l, base, am2, W);
+#pragma unroll
+                        for (int b = 0; b < B; ++b)
+#pragma unroll
+                            for (int c = 0; c < 3; ++c) KL[i][b][c] = K6[b][c];
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 1; i < 6; ++i) {  // stages 2 .. 6
+                        const double ch = q.c[i] * h;
+#pragma unroll
+                        for (int b = 0; b < B; ++b)
+#pragma unroll
+                            for (int c = 0; c < 3; ++c) {
+                                double s = 0.0;
+#pragma unroll
+                                for (int ll = 0; ll + 2 <= i; ++ll) s = fma(q.AA[i][ll], K[ll][b][c], s);
+                                Xs[b][c] = fma(h2, s, fma(ch, V[b][c], X[b][c]));
+                            }
+                        if (i < 5)
+                            eval_acc_planets<N, L, B>(Xs, m, K[i], dummy, l, base, am2, W);
+                        else
+                            eval_acc_planets<N, L, B>(Xs, m, K6, dummy, l, base, am2, W);
+                    }
                 }
+                // the stage accelerations the sums below read: registers, or the local-memory copy
+                auto& KK = *[&] {
+                    if constexpr (ROLLED) return &KL;
+                    else return &K;
+                }();
                 // error level of this trial (scales from the state the step starts from)
                 double ex = 0.0, ev = 0.0, x2 = 0.0, v2 = 0.0;
 #pragma unroll
@@ -469,11 +508,11 @@ __global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkU
                         for (int c = 0; c < 3; ++c) {
                             double sx = 0.0;
 #pragma unroll
-                            for (int ll = 0; ll < 5; ++ll) sx = fma(q.dA[ll], K[ll][b][c], sx);
-                            double sv = q.d[0] * K[0][b][c];  // d_2 = 0
-                            sv = fma(q.d[2], K[2][b][c], sv);
-                            sv = fma(q.d[3], K[3][b][c], sv);
-                            sv = fma(q.d[4], K[4][b][c], sv);
+                            for (int ll = 0; ll < 5; ++ll) sx = fma(q.dA[ll], KK[ll][b][c], sx);
+                            double sv = q.d[0] * KK[0][b][c];  // d_2 = 0
+                            sv = fma(q.d[2], KK[2][b][c], sv);
+                            sv = fma(q.d[3], KK[3][b][c], sv);
+                            sv = fma(q.d[4], KK[4][b][c], sv);
                             sv = fma(q.d[5], K6[b][c], sv);
                             ex = fmax(ex, fabs(sx));
                             ev = fmax(ev, fabs(sv));
@@ -508,11 +547,11 @@ __global__ void __maxnreg__(MAXREG) rkck_adaptive_kernel(View e, StepArgs p, RkU
                         for (int c = 0; c < 3; ++c) {
                             double s = 0.0;
 #pragma unroll
-                            for (int ll = 0; ll < 5; ++ll) s = fma(q.bA[ll], K[ll][b][c], s);
+                            for (int ll = 0; ll < 5; ++ll) s = fma(q.bA[ll], KK[ll][b][c], s);
                             X[b][c] = fma(h2, s, fma(h, V[b][c], X[b][c]));
-                            double w = q.b[0] * K[0][b][c];  // b_2 = b_5 = 0
-                            w = fma(q.b[2], K[2][b][c], w);
-                            w = fma(q.b[3], K[3][b][c], w);
+                            double w = q.b[0] * KK[0][b][c];  // b_2 = b_5 = 0
+                            w = fma(q.b[2], KK[2][b][c], w);
+                            w = fma(q.b[3], KK[3][b][c], w);
                             w = fma(q.b[5], K6[b][c], w);
                             V[b][c] = fma(h, w, V[b][c]);
                         }
