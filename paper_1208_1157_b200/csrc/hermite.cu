@@ -47,11 +47,15 @@ ENS_SHAPE(6, 1, 6, 2, 32, 1, 32)
 // 336 / 688 B) and are 3 - 4 % faster.
 ENS_SHAPE(7, 1, 7, 2, 32, 1, 32)
 ENS_SHAPE(8, 1, 8, 2, 32, 1, 32)
-ENS_SHAPE(9, 3, 3, 0, 64, 1, 128)
+// n_body = 9 .. 12: the evaluation of these shapes is small enough (12 / 9 / 22 pairs per lane) for a straight-line step:
+// three copies at n = 9, 10 (+5 %, +3 % at 32768 systems; n = 10 at 131072 systems, the paper's largest Table 3 shape:
+// 0.617 -> 0.664), two at n = 11, 12 (+2 .. 3 %); the 5 x 3 shapes (n >= 13) stay on the 3-phase loop (three copies:
+// 0.54 against 0.64 on config 3)
+ENS_SHAPE(9, 3, 3, 1, 64, 1, 128)
 // n_body = 10 (the paper's largest Table 3 shape): 168 registers -> 12 warps per SM: 0.60 against 0.54 at 242 registers
-ENS_SHAPE(10, 5, 2, 0, 64, 3, 128)
-ENS_SHAPE(11, 3, 4, 0, 64, 1, 128)
-ENS_SHAPE(12, 3, 4, 0, 64, 1, 128)
+ENS_SHAPE(10, 5, 2, 1, 64, 3, 128)
+ENS_SHAPE(11, 3, 4, 2, 64, 1, 128)
+ENS_SHAPE(12, 3, 4, 2, 64, 1, 128)
 ENS_SHAPE(13, 5, 3, 0, 64, 1, 128)
 ENS_SHAPE(14, 5, 3, 0, 64, 1, 128)
 ENS_SHAPE(15, 5, 3, 0, 64, 1, 128)
@@ -60,6 +64,15 @@ ENS_SHAPE(16, 5, 4, 0, 64, 1, 128)
 ENS_SHAPE_MODE(3, 2, 1, 64, 5, 64)
 // n_body = 6 with carried a, j: the straight-line step spilled 464 B; the 3-phase loop spills 16 B and is 3.7 % faster
 ENS_SHAPE_MODE(6, 2, 0, 32, 1, 32)
+// the adaptive and the 2-evaluation kernels of the many-lane shapes keep the 3-phase loop
+ENS_SHAPE_MODE(9, 1, 0, 64, 1, 128)
+ENS_SHAPE_MODE(9, 2, 0, 64, 1, 128)
+ENS_SHAPE_MODE(10, 1, 0, 64, 3, 128)
+ENS_SHAPE_MODE(10, 2, 0, 64, 3, 128)
+ENS_SHAPE_MODE(11, 1, 0, 64, 1, 128)
+ENS_SHAPE_MODE(11, 2, 0, 64, 1, 128)
+ENS_SHAPE_MODE(12, 1, 0, 64, 1, 128)
+ENS_SHAPE_MODE(12, 2, 0, 64, 1, 128)
 #undef ENS_SHAPE
 #undef ENS_SHAPE_MODE
 
