@@ -12,7 +12,7 @@ template <int N> struct RkShape;
 #define ENS_RK_SHAPE_A(N_, L_, B_, THREADS_, MAXREG_, MAXREG_A_)                                         \
     template <> struct RkShape<N_> {                                                                     \
         static constexpr int L = L_, B = B_, THREADS = THREADS_, MAXREG = MAXREG_, MAXREG_A = MAXREG_A_; \
-        static constexpr bool ROLLED = (N_ == 7) || (L_ == 5 && B_ >= 3) || (L_ == 3 && B_ >= 4); /* stages 2 .. 6 as a loop (rkck_kernel.cuh) */ \
+        static constexpr bool ROLLED = (N_ == 6 || N_ == 7) || (L_ == 5 && B_ >= 3) || (L_ == 3 && B_ >= 4); /* stages 2 .. 6 as a loop (rkck_kernel.cuh) */ \
     };
 #define ENS_RK_SHAPE(N_, L_, B_, THREADS_, MAXREG_) ENS_RK_SHAPE_A(N_, L_, B_, THREADS_, MAXREG_, MAXREG_)
 //           N   L  B  threads maxRegisters
@@ -23,7 +23,9 @@ ENS_RK_SHAPE(4, 1, 4, 64, 255)
 // n_body = 5, 7: one system per thread with part of the stage accelerations in local memory (344 / 1448 B, L1-resident)
 // beats the padded lane-split shapes: 9.0e9 against 5.0e9 and 2.5e9 against 2.1e9 system-steps/s
 ENS_RK_SHAPE(5, 1, 5, 32, 255)
-ENS_RK_SHAPE(6, 3, 2, 64, 255)
+// n_body = 6: one system per thread with the rolled stage loop (864 B of stage accelerations in local memory): 5.63e9
+// against 5.30e9 system-steps/s for 3 lanes x 2 bodies
+ENS_RK_SHAPE(6, 1, 6, 32, 255)
 ENS_RK_SHAPE(7, 1, 7, 32, 255)
 ENS_RK_SHAPE(8, 3, 3, 64, 255)
 ENS_RK_SHAPE(9, 3, 3, 64, 255)
