@@ -45,7 +45,10 @@ extern "C" {
 
 typedef struct ens ens_t; /* opaque */
 
-enum { ENS_OK = 0, ENS_EINVAL = -1, ENS_ENOMEM = -2, ENS_ECUDA = -3, ENS_ESTATE = -4, ENS_EUNSUPPORTED = -5 };
+enum {
+    ENS_OK = 0, ENS_EINVAL = -1, ENS_ENOMEM = -2, ENS_ECUDA = -3, ENS_ESTATE = -4, ENS_EUNSUPPORTED = -5,
+    ENS_ETOOLARGE = -6 /* ens_hermite_static: the ensemble needs more than the library's static scratch holds */
+};
 enum {
     ENS_HERMITE = 0, ENS_MVS = 1, ENS_HERMITE_ADAPTIVE = 2, ENS_HERMITE_CARRY = 3, ENS_RKCK = 4,
     ENS_MVS_MERGED = 5,    /* MVS with the adjacent half sub-steps of consecutive steps merged */
@@ -160,6 +163,33 @@ ENS_API int ens_log_read(const ens_t *e, int64_t *n_records, int64_t *n_dropped,
  * L != NULL, total angular momentum sum m x cross v, per system, computed on the device ("only 1-4 values
  * per system need to be transferred").  EINVAL: NULL e or E.  ESTATE: no state was set. */
 ENS_API int ens_energy(const ens_t *e, double *E, double *L, int memspace, void *stream);
+
+/* The fixed-step Hermite step loop of ens_integrate(ENS_HERMITE) WITHOUT A HANDLE AND WITHOUT ANY ALLOCATION, for
+ * callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+ * no cudaMalloc, cudaFree or allocating library routine is called, here or in anything this calls.
+ * The caller owns the ensemble, as DEVICE arrays in the library's structure-of-arrays layout, all
+ * advanced in place:  pos, vel [n_body * 3][n_pad] (row = body * 3 + component, n_pad >= n_sys consecutive systems
+ * per row);  mass [n_body][n_pad] (read only);  time [n_pad];  status int32 [n_pad] (ENS_ACTIVE = 0 to start a system;
+ * the status semantics of ens_integrate: DONE_* run again, STOP_* are skipped);  nsteps int64 [n_pad] (the steps
+ * taken are ADDED to it).  Columns n_sys .. n_pad - 1 are never touched.  dt, t_end, max_steps as in ens_integrate;
+ * r_close, r_eject as in ens_set_monitors (<= 0 switches that monitor off).  Results are bit-identical to
+ * ens_integrate(ENS_HERMITE) on the same state (the step is a pure function of the state, reading R6).
+ * The kernel is the time-sliced persistent grid; its scratch (a task counter and one int32
+ * progress word per warp-group of 32 / L systems, L = lanes per system: 1 for n_body <= 8, 3 or 5 above) is a
+ * file-scope device array of ENS_STATIC_MAX_GROUPS words + 256 bytes = 256.25 KB that every GPU which loads the
+ * library holds until the process exits.  Limit: ceil(n_sys / (32 / L)) <= ENS_STATIC_MAX_GROUPS, i.e. at most
+ * 2097152 systems of n_body <= 8, 655360 of 9..12 bodies (393216 of 10), 393216 of 13..16; beyond it ETOOLARGE.
+ * ALL calls on one device share that array and each finds the last call's contents in it: the words a launch uses are
+ * cleared on `stream` right before its kernel, so calls ordered on one stream (or by events) are safe, and two calls
+ * that OVERLAP on the GPU race on it (undefined results).  The first call on a device looks the array's device
+ * address up (cudaGetSymbolAddress, with that device current) and loads the module: make it outside graph capture.
+ * Runs on the CURRENT device; only enqueues on `stream` and returns.
+ * EINVAL: NULL pointer, n_sys < 1, n_pad < n_sys, n_body outside 2..16, dt == 0 or non-finite, NaN t_end / r_close /
+ * r_eject, max_steps < 0.  ETOOLARGE: see above.  ECUDA: no device / lookup or launch failed. */
+#define ENS_STATIC_MAX_GROUPS 65536
+ENS_API int ens_hermite_static(double *pos, double *vel, const double *mass, double *time, int32_t *status,
+                               int64_t *nsteps, int64_t n_sys, int64_t n_pad, int n_body, double dt, double t_end,
+                               int64_t max_steps, double r_close, double r_eject, void *stream);
 
 /* Static description of an error code; for ENS_ECUDA the text of the last CUDA error seen by this thread. */
 ENS_API const char *ens_strerror(int code);

@@ -24,6 +24,15 @@ int cuda_fail(cudaError_t err, const char* what) {
         if (err__ != cudaSuccess) return cuda_fail(err__, #call); \
     } while (0)
 
+}  // namespace
+
+namespace ensd {
+// for the translation units that hold other entry points (hermite_static.cu): same error text channel
+int record_cuda_error(cudaError_t err, const char* what) { return cuda_fail(err, what); }
+}  // namespace ensd
+
+namespace {
+
 constexpr int TILE = 64;  // systems per transposition tile = padding granule of the SoA rows
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -389,6 +398,9 @@ const char* ens_strerror(int code) {
         case ENS_ECUDA: return g_cuda_err;
         case ENS_ESTATE: return "no state set (call ens_set_state first)";
         case ENS_EUNSUPPORTED: return "unsupported configuration";
+        case ENS_ETOOLARGE:
+            return "ensemble too large for the static scratch (ens_hermite_static: more than ENS_STATIC_MAX_GROUPS = 65536 "
+                   "warp-groups of systems; use a handle, ens_create + ens_integrate)";
         default: return "unknown error code";
     }
 }

@@ -12,7 +12,8 @@ import os
 import numpy as np
 import torch
 
-OK, EINVAL, ENOMEM, ECUDA, ESTATE, EUNSUPPORTED = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ENOMEM, ECUDA, ESTATE, EUNSUPPORTED, ETOOLARGE = 0, -1, -2, -3, -4, -5, -6
+STATIC_MAX_GROUPS = 65536  # ens_hermite_static: warp-groups of systems its static scratch holds (include/ens.h)
 # HERMITE_ADAPTIVE: `dt` is the step size scale tau of Eq. 5; RKCK_ADAPTIVE: `dt` is the first trial step
 HERMITE, MVS, HERMITE_ADAPTIVE, HERMITE_CARRY, RKCK, MVS_MERGED, RKCK_ADAPTIVE = 0, 1, 2, 3, 4, 5, 6
 HOST, DEVICE = 0, 1
@@ -27,7 +28,7 @@ SYMBOLS = (
     "ens_create", "ens_destroy", "ens_set_state", "ens_set_monitors", "ens_integrate", "ens_get_state",
     "ens_energy", "ens_strerror", "ens_get_info", "ens_last_kernel_ms", "ens_fp64_peak", "ens_test_rsqrt",
     "ens_test_rcp", "ens_log_enable", "ens_integrate_logged", "ens_log_read", "ens_reserve_host_staging",
-    "ens_test_set_option", "ens_set_rk_tolerance", "ens_get_rejected",
+    "ens_test_set_option", "ens_set_rk_tolerance", "ens_get_rejected", "ens_hermite_static",
 )
 _lib = None
 
@@ -76,6 +77,7 @@ def lib() -> ctypes.CDLL:
         L.ens_set_rk_tolerance.argtypes = [vp, cd]
         L.ens_get_rejected.argtypes = [vp, vp, ci, vp]
         L.ens_test_set_option.argtypes = [vp, ci, i64]
+        L.ens_hermite_static.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, ci, cd, cd, i64, cd, cd, vp]
         L.ens_log_read.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64), vp, vp, vp, vp, vp, vp, i64, ci, vp]
         for name in SYMBOLS:
             if name != "ens_strerror":
@@ -255,6 +257,24 @@ class Ensemble:
         ms = ctypes.c_float()
         _check(lib().ens_last_kernel_ms(self._h, ctypes.byref(ms)), "ens_last_kernel_ms")
         return ms.value
+
+
+def hermite_static(pos, vel, mass, time, status, nsteps, n_sys: int, n_body: int, dt: float, max_steps: int,
+                   t_end: float = float("inf"), r_close: float = 0.0, r_eject: float = float("inf"), stream=None):
+    """``ens_hermite_static``: the fixed-step Hermite loop on caller-owned CUDA tensors in the library's SoA layout
+    (pos, vel [n_body * 3][n_pad], mass [n_body][n_pad], time, status int32, nsteps int64 [n_pad]), advanced in place;
+    the library allocates nothing (its scratch is a static device array shared by all calls: keep calls stream-ordered)."""
+    n_pad = int(time.numel())
+    ptrs = []
+    for a, dt_, cnt, what in ((pos, np.float64, n_body * 3 * n_pad, "pos"), (vel, np.float64, n_body * 3 * n_pad, "vel"),
+                              (mass, np.float64, n_body * n_pad, "mass"), (time, np.float64, n_pad, "time"),
+                              (status, np.int32, n_pad, "status"), (nsteps, np.int64, n_pad, "nsteps")):
+        ptr, space, _ = _ptr(a, dt_, cnt, what)
+        if space != DEVICE:
+            raise ValueError(f"ens_hermite_static: {what} must be a CUDA tensor")
+        ptrs.append(ptr)
+    _check(lib().ens_hermite_static(*ptrs, int(n_sys), n_pad, int(n_body), float(dt), float(t_end), int(max_steps),
+                                    float(r_close), float(r_eject), _stream_ptr(stream)), "ens_hermite_static")
 
 
 def fp64_peak(iters: int = 200000, stream=None) -> float:
