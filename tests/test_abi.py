@@ -49,6 +49,34 @@ def test_strerror_and_argument_checks_need_no_gpu(libpath):
     assert lib.ens_create(ctypes.c_int64(8), 99, ctypes.byref(h)) == -1
 
 
+def test_static_entry_point_checks_sizes_before_any_cuda_call(libpath):
+    """ens_hermite_static: argument errors and the size limit of its static scratch are decided on the host, before the
+    first CUDA call (so they are testable here); the limit is ENS_STATIC_MAX_GROUPS warp-groups of 32 / L systems."""
+    lib = ctypes.CDLL(libpath)
+    vp, i64, ci, cd = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double
+    lib.ens_hermite_static.argtypes = [vp, vp, vp, vp, vp, vp, i64, i64, ci, cd, cd, i64, cd, cd, vp]
+    lib.ens_strerror.restype = ctypes.c_char_p
+    text = open(os.path.join(ROOT, "include", "ens.h")).read()
+    max_groups = int(re.search(r"#define\s+ENS_STATIC_MAX_GROUPS\s+(\d+)", text).group(1))
+    from paper_1208_1157_b200 import ens
+    assert max_groups == ens.STATIC_MAX_GROUPS and ens.ETOOLARGE == -6
+    buf = (ctypes.c_double * 8)()
+    p = ctypes.addressof(buf)  # never dereferenced: every call below returns before touching memory
+
+    def call(n_sys, n_pad, n_body, dt=0.01, t_end=float("inf"), steps=10, first=p):
+        return lib.ens_hermite_static(first, p, p, p, p, p, n_sys, n_pad, n_body, dt, t_end, steps, 0.0, float("inf"), None)
+
+    assert call(8, 8, 3, first=None) == -1
+    assert call(0, 8, 3) == -1 and call(9, 8, 3) == -1 and call(8, 8, 1) == -1 and call(8, 8, 17) == -1
+    assert call(8, 8, 3, dt=0.0) == -1 and call(8, 8, 3, dt=float("nan")) == -1 and call(8, 8, 3, t_end=float("nan")) == -1
+    assert call(8, 8, 3, steps=-1) == -1
+    # lanes per system: 1 up to 8 bodies, 3 for 9, 11, 12, 5 for 10 and 13..16 -> systems per warp-group 32, 10, 6
+    for n_body, per_group in ((2, 32), (8, 32), (9, 10), (10, 6), (11, 10), (12, 10), (13, 6), (16, 6)):
+        n = max_groups * per_group + 1
+        assert call(n, n, n_body) == -6, n_body
+    assert b"static scratch" in lib.ens_strerror(-6)
+
+
 def test_no_cpu_fallback_without_device(libpath):
     import torch
     if torch.cuda.is_available():
