@@ -125,9 +125,23 @@ cudaError_t launch_n(const View& v, StepArgs a, const LaunchTune& tune, cudaStre
     const int wpb = threads / 32;
     int64_t blocks = (warps + wpb - 1) / wpb;
     cudaError_t err = cudaSuccess;
-    if constexpr (MODE == 1) {  // persistent grid: what the device holds at once; lane groups pull systems from a.counter
-        int64_t resident = 0;
+    if constexpr (MODE == 1) {  // persistent grid; lane groups pull systems from a.counter
+        int64_t resident = 0;  // what the device holds at once
         if ((err = resident_blocks<N, MODE>(threads, &resident)) != cudaSuccess) return err;
+        // Systems take different numbers of steps (config 1: the longest 2.2 x the mean), each is a serial chain, and the
+        // launch ends with the last one: what counts is systems per lane group (the longest-first hand-out balances only
+        // when every group gets several), not resident warps.  Measured: two warps per SM
+        // sub-partition are never slower than four (n_body = 3: 131072 systems +11 %, 524288 +1 %); one-system-per-thread
+        // shapes with fewer than 1.5 systems per lane of such a grid run faster on one warp per sub-partition (n_body = 3,
+        // 32768 systems: +17 %; n_body = 6: +53 %), the many-lane shapes do not (a lone warp cannot hide its ring).
+        int dev = 0, sms = 0;
+        if ((err = cudaGetDevice(&dev)) != cudaSuccess) return err;
+        if ((err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return err;
+        const int64_t per_sm = resident / sms;
+        const int64_t g = wpb >= 4 ? 1 : 4 / wpb;  // blocks per SM that give every sub-partition one warp
+        int64_t k = 2;
+        if (S::L == 1 && 2 * v.n_sys < 3 * ((int64_t)sms * 2 * g * threads)) k = 1;
+        if (k * g < per_sm) resident = k * g * sms;
         if (blocks > resident) blocks = resident;
     }
     if constexpr (MODE == 0) {
